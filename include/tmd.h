@@ -1,0 +1,169 @@
+/*
+ * tmd.h -- C ABI of the B200-native TPC track-model decoder (libtmd.so).
+ *
+ * The operation is the one arXiv:2411.02206 describes in §4:
+ *   L68  "after the entropy decoding, the clusters' coordinates must be decoded to the absolute values instead of
+ *         residuals or differences" -- input = the entropy-decoded compressed-cluster arrays, output = clusters;
+ *   L70  attached clusters: "every GPU-thread receives one track, it propagates it through the TPC and computes the
+ *         absolute values of the coordinates using the residuals given in input and the reconstructed track";
+ *         unattached clusters: "computes each coordinate summing the difference taken from the input array with the
+ *         coordinates of the last decoded cluster; each thread decodes clusters from a specific region of the TPC";
+ *         the input is a "Structure Of Arrays (SOA)".
+ * The paper fixes no layout, geometry, quantisation or output order; those are the readings in DESIGN.md §3
+ * (model = SURVEY.md §8(c) C1-C5).  Step names A1..A7 below are the rows of SURVEY.md §8(a).
+ *
+ * Conventions for every function:
+ *   - returns TMD_OK (0) or a negative tmd_status; never throws, aborts or prints;
+ *   - "HOST" / "DEVICE" says in which address space a pointer lives;
+ *   - the library owns only tmd_ctx; all data buffers, outputs and the workspace belong to the caller.
+ */
+#ifndef TMD_H_
+#define TMD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  TMD_OK = 0,
+  TMD_ERR_ARG = -1,       /* null pointer, size out of the limits below, bad geometry                         */
+  TMD_ERR_ALIGN = -2,     /* a device pointer is not aligned as required                                     */
+  TMD_ERR_WORKSPACE = -3, /* workspace missing or smaller than tmd_workspace_bytes()                         */
+  TMD_ERR_CUDA = -4,      /* a CUDA runtime call failed (allocation, copy, launch)                           */
+  TMD_ERR_CORRUPT = -5    /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
+} tmd_status;
+
+/* Limits: n_attached + n_unattached < 2^32; trk_ncl in [1, 65535]; n_rows <= 255; n_az <= 63; n_sides in {1,2};
+ * n_sectors_out <= n_az * n_sides; n_sectors_out * n_rows <= 8192. */
+
+/* Pad-plane geometry (DESIGN.md §3 reading 1).  HOST pointers; deep-copied by tmd_create. */
+typedef struct {
+  uint32_t n_az;           /* azimuthal sectors per side (18)                                                  */
+  uint32_t n_sides;        /* 2; sector = side * n_az + az                                                     */
+  uint32_t n_sectors_out;  /* sectors that own output bins: 36, or 2 for the tiny config (sectors 0,1)         */
+  uint32_t n_rows;         /* pad rows per sector (152)                                                        */
+  float cos_a, sin_a;      /* cos / sin of the sector angle (20 deg) as binary32                               */
+  const float* row_x;        /* [n_rows] cm, x of the pad row in the sector frame                              */
+  const float* row_padw;     /* [n_rows] cm, pad width                                                         */
+  const float* row_inv_padw; /* [n_rows] 1/cm, binary32 of the double reciprocal                               */
+  const uint16_t* row_npads; /* [n_rows] pads in the row (even)                                                */
+} tmd_geometry;
+
+typedef struct {
+  float bz_tesla;          /* solenoid field; the curvature unit is KB = bz_tesla * 0.00299792458f             */
+} tmd_field;
+
+/*
+ * Compressed-cluster SoA of one time frame ("input Structure Of Arrays"; layout DESIGN.md §3 / SURVEY C2).
+ * All arrays: DEVICE pointers in tmd_decode (HOST pointers in tmd_decode_host), caller-owned, read-only for the
+ * library, each aligned to 16 bytes.  Little endian.  Arrays of length 0 may be null.
+ *   off[t]  = sum of trk_ncl[0..t)   (computed by the library, A1; the paper precomputes these indices on the CPU, L70)
+ *   per track t, cluster j = 0 is stored absolute; cluster j >= 1 uses residual index  off[t] - t + j - 1.
+ */
+typedef struct {
+  uint32_t n_tracks;
+  uint64_t n_attached;     /* = sum trk_ncl                                                                    */
+  uint64_t n_unattached;   /* = sum u_bin_count                                                                */
+  /* per track [n_tracks] */
+  const uint16_t* trk_ncl;   /* clusters on the track, >= 1                                                    */
+  const int8_t* trk_qpt;     /* q/pT in 1/16 c/GeV                                                             */
+  const uint8_t* trk_row0;   /* first cluster: pad row, sector, pad code (pad*64), time code (bin*64)          */
+  const uint8_t* trk_sec0;
+  const uint16_t* trk_pad0;
+  const uint32_t* trk_time0;
+  /* per attached cluster incl. the first of each track [n_attached], index g = off[t] + j; copied through        */
+  const uint16_t* a_qtot;
+  const uint16_t* a_qmax;
+  const uint8_t* a_flags;
+  const uint8_t* a_sigpad;
+  const uint8_t* a_sigtime;
+  /* per attached cluster excl. the first of each track [n_attached - n_tracks]                                   */
+  const uint8_t* a_rowdiff;   /* (row - row_prev) * dir  mod n_rows  (values are reduced mod n_rows)             */
+  const uint8_t* a_secleg;    /* bit 7: leg change; bits 0-5: (az - az_prev) mod n_az (reduced mod n_az); bit 6 ignored */
+  const uint16_t* a_padres;   /* (P - P_pred) mod 2^16                                                           */
+  const uint32_t* a_timeres;  /* (T - T_pred) mod 2^32                                                           */
+  /* per unattached cluster [n_unattached], bin after bin in bin order                                            */
+  const uint16_t* u_qtot;
+  const uint16_t* u_qmax;
+  const uint8_t* u_flags;
+  const uint8_t* u_sigpad;
+  const uint8_t* u_sigtime;
+  const uint16_t* u_paddiff;  /* difference to the preceding cluster of the bin, mod 2^16 (first: to 0)          */
+  const uint32_t* u_timediff; /* same for time, mod 2^32                                                         */
+  const uint32_t* u_bin_count; /* [n_sectors_out * n_rows] unattached clusters per bin = sector * n_rows + row   */
+} tmd_compressed;
+
+/* One decoded cluster: 16 bytes, little endian, naturally aligned. */
+typedef struct {
+  uint32_t time;   /* time code T = time bin * 64                                                              */
+  uint16_t pad;    /* pad code  P = pad * 64                                                                   */
+  uint16_t qtot;
+  uint16_t qmax;
+  uint8_t sigpad;
+  uint8_t sigtime;
+  uint8_t flags;
+  uint8_t row;
+  uint8_t sector;
+  uint8_t zero;    /* always 0                                                                                 */
+} tmd_cluster;
+
+/*
+ * Output (DEVICE pointers in tmd_decode, HOST pointers in tmd_decode_host; caller-owned, written by the library).
+ * Canonical order (DESIGN.md §3 reading 11): bin b = sector * n_rows + row owns clusters[bin_offset[b] .. bin_offset[b+1]):
+ * first the attached clusters of the bin in ascending global attached index g, then its unattached clusters in
+ * stored order.
+ */
+typedef struct {
+  tmd_cluster* clusters;   /* [n_attached + n_unattached], 16-byte aligned                                     */
+  uint32_t* bin_offset;    /* [n_sectors_out * n_rows + 1]                                                     */
+  uint32_t* probe_state;   /* nullable: [n_tracks][6] binary32 bit patterns of the track state (x,y,u,sp,dt,k)
+                              after cluster min(probe_step, trk_ncl-1) has been rebuilt and the state updated  */
+  uint32_t probe_step;     /* UINT32_MAX = final state                                                         */
+  void* workspace;         /* DEVICE scratch, 256-byte aligned; ignored by tmd_decode_host                     */
+  size_t workspace_bytes;  /* >= tmd_workspace_bytes(...)                                                      */
+} tmd_output;
+
+typedef struct tmd_ctx tmd_ctx;
+
+/* flags of tmd_decode */
+#define TMD_VALIDATE 1u /* check on the device that sum(trk_ncl) == n_attached, sum(u_bin_count) == n_unattached,
+                           every trk_ncl >= 1, trk_row0 < n_rows, trk_sec0 < n_az*n_sides and every decoded sector
+                           < n_sectors_out; synchronises the stream; returns TMD_ERR_CORRUPT on failure.
+                           Without it such inputs are undefined except that nothing is written out of bounds
+                           of `clusters` for a decoded sector >= n_sectors_out (the cluster is dropped). */
+
+/* Uploads the geometry tables to the current CUDA device.  *out_ctx is set only on success. */
+int tmd_create(const tmd_geometry* geometry, const tmd_field* field, tmd_ctx** out_ctx);
+
+/* Scratch bytes tmd_decode needs for a time frame of this size (a pure function of the sizes). */
+int tmd_workspace_bytes(const tmd_ctx* ctx, uint32_t n_tracks, uint64_t n_attached, uint64_t n_unattached, size_t* out_bytes);
+
+/*
+ * Decode one time frame (rows A1-A7).  Only enqueues kernels on `cuda_stream` (a cudaStream_t; null = default stream)
+ * and returns; no allocation, no host synchronisation and no device-to-host copy unless TMD_VALIDATE is set.
+ * Results are valid once the stream has been synchronised.  Concurrent calls need distinct workspaces.
+ */
+int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream);
+
+/*
+ * End-to-end convenience: every pointer in `in` / `out` is a HOST pointer (pinned memory makes the copies asynchronous;
+ * out->workspace is ignored).  Copies the inputs to device buffers owned by the context (grown on demand and reused),
+ * runs tmd_decode, copies clusters / bin_offset / probe_state back and synchronises the stream.
+ */
+int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream);
+
+/* Frees the context and its device tables / buffers.  Null is accepted. */
+int tmd_destroy(tmd_ctx* ctx);
+
+const char* tmd_status_string(int status);
+
+/* Number of kernel launches the last tmd_decode on this context enqueued (for bench.py's gpu_launches). */
+int tmd_last_launch_count(const tmd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TMD_H_ */

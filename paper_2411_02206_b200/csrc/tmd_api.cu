@@ -1,0 +1,338 @@
+// tmd_api.cu -- the C ABI of libtmd.so (include/tmd.h): context, workspace layout, kernel sequencing.
+// Every step of the path runs in the kernels of this directory; the host code only checks arguments and enqueues.
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+#include "tmd_common.cuh"
+#include "tmd_decode.cuh"
+#include "tmd_rank.cuh"
+#include "tmd_scan.cuh"
+#include "tmd_unattached.cuh"
+
+using namespace tmd;
+
+struct tmd_ctx {
+  DevGeo geo;
+  RowGeo* d_rows;
+  int device;
+  int launches;
+  // arena of tmd_decode_host (grown on demand)
+  void* arena;
+  size_t arena_bytes;
+};
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
+
+struct Workspace {
+  uint32_t n_tiles, n_chunks, n_groups;
+  size_t o_err, o_tile_sum, o_off, o_chunk_first, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, total;
+};
+
+Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
+  Workspace w;
+  w.n_tiles = (n_tracks + SCAN_TILE - 1) / SCAN_TILE;
+  w.n_chunks = (uint32_t)((n_att + CHUNK_WINDOW - 1) >> CHUNK_SHIFT);
+  w.n_groups = (w.n_chunks + COL_GROUP - 1) / COL_GROUP;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
+  w.o_err = take(ERR_WORDS * 4);
+  w.o_tile_sum = take(((size_t)w.n_tiles + 1) * 4);
+  w.o_off = take(((size_t)n_tracks + 1) * 4);
+  w.o_chunk_first = take(((size_t)w.n_chunks + 1) * 4);
+  w.o_att_cnt = take((size_t)n_bins * 4);
+  w.o_u_start = take(((size_t)n_bins + 1) * 4);
+  w.o_gsum = take((size_t)w.n_groups * n_bins * 4);
+  w.o_hist = take((size_t)w.n_chunks * n_bins * 2);
+  w.o_rel = take((size_t)w.n_chunks * n_bins * 4);
+  w.o_rank16 = take((size_t)n_att * 2);
+  w.total = o;
+  return w;
+}
+
+inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+
+// TMD_VALIDATE, part 1 (before anything indexes with the counts): per-track fields and the two totals.
+__global__ void k_validate(DevGeo G, tmd_compressed in, const uint32_t* __restrict__ off, uint32_t* __restrict__ err) {
+  __shared__ unsigned long long s_sum;
+  if (threadIdx.x == 0) s_sum = 0;
+  __syncthreads();
+  uint32_t bad = 0;
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < in.n_tracks; t += gridDim.x * blockDim.x)
+    bad |= (in.trk_ncl[t] < 1) | (in.trk_row0[t] >= G.n_rows) | (in.trk_sec0[t] >= G.n_az * G.n_sides);
+  if (bad) atomicOr(&err[ERR_TRACK_FIELD], 1u);
+  if (blockIdx.x == 0) {
+    unsigned long long s = 0;
+    for (uint32_t b = threadIdx.x; b < G.n_bins; b += blockDim.x) s += in.u_bin_count[b];
+    atomicAdd(&s_sum, s);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      if (s_sum != in.n_unattached) atomicOr(&err[ERR_TRACK_FIELD], 2u);
+      if (in.n_tracks > 0 && off[in.n_tracks] != (uint32_t)in.n_attached) atomicOr(&err[ERR_TRACK_FIELD], 4u);
+    }
+  }
+}
+
+int check_args(const tmd_ctx* ctx, const tmd_compressed* in, const tmd_output* out, bool device_side) {
+  if (!ctx || !in || !out) return TMD_ERR_ARG;
+  if (in->n_attached + in->n_unattached >= (1ull << 32)) return TMD_ERR_ARG;
+  if (in->n_attached < in->n_tracks) return TMD_ERR_ARG;
+  if ((in->n_tracks == 0) != (in->n_attached == 0)) return TMD_ERR_ARG;
+  const bool has_trk = in->n_tracks > 0, has_res = in->n_attached > in->n_tracks, has_un = in->n_unattached > 0;
+  const void* trk[] = {in->trk_ncl, in->trk_qpt, in->trk_row0, in->trk_sec0, in->trk_pad0, in->trk_time0,
+                       in->a_qtot, in->a_qmax, in->a_flags, in->a_sigpad, in->a_sigtime};
+  const void* res[] = {in->a_rowdiff, in->a_secleg, in->a_padres, in->a_timeres};
+  const void* un[] = {in->u_qtot, in->u_qmax, in->u_flags, in->u_sigpad, in->u_sigtime, in->u_paddiff, in->u_timediff};
+  for (const void* p : trk) if (has_trk && !p) return TMD_ERR_ARG;
+  for (const void* p : res) if (has_res && !p) return TMD_ERR_ARG;
+  for (const void* p : un) if (has_un && !p) return TMD_ERR_ARG;
+  if (!in->u_bin_count || !out->bin_offset) return TMD_ERR_ARG;
+  if ((in->n_attached + in->n_unattached) > 0 && !out->clusters) return TMD_ERR_ARG;
+  if (device_side) {
+    for (const void* p : trk) if (has_trk && misaligned(p, 16)) return TMD_ERR_ALIGN;
+    for (const void* p : res) if (has_res && misaligned(p, 16)) return TMD_ERR_ALIGN;
+    for (const void* p : un) if (has_un && misaligned(p, 16)) return TMD_ERR_ALIGN;
+    if (misaligned(in->u_bin_count, 16) || misaligned(out->clusters, 16) || misaligned(out->bin_offset, 4) ||
+        misaligned(out->probe_state, 4))
+      return TMD_ERR_ALIGN;
+  }
+  return TMD_OK;
+}
+
+#define TMD_LAUNCH_CHECK()                           \
+  do {                                               \
+    ctx->launches++;                                 \
+    if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA; \
+  } while (0)
+
+}  // namespace
+
+extern "C" {
+
+int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
+  if (!g || !f || !out_ctx) return TMD_ERR_ARG;
+  if (!g->row_x || !g->row_padw || !g->row_inv_padw || !g->row_npads) return TMD_ERR_ARG;
+  if (g->n_az < 1 || g->n_az > 63 || g->n_sides < 1 || g->n_sides > 2 || g->n_rows < 1 || g->n_rows > 255) return TMD_ERR_ARG;
+  if (g->n_sectors_out < 1 || g->n_sectors_out > g->n_az * g->n_sides) return TMD_ERR_ARG;
+  if ((uint64_t)g->n_sectors_out * g->n_rows > MAX_BINS) return TMD_ERR_ARG;
+  tmd_ctx* ctx = new (std::nothrow) tmd_ctx();
+  if (!ctx) return TMD_ERR_CUDA;
+  memset(ctx, 0, sizeof(*ctx));
+  if (cudaGetDevice(&ctx->device) != cudaSuccess) { delete ctx; return TMD_ERR_CUDA; }
+  RowGeo* h = (RowGeo*)malloc(sizeof(RowGeo) * g->n_rows);
+  if (!h) { delete ctx; return TMD_ERR_CUDA; }
+  for (uint32_t r = 0; r < g->n_rows; ++r) {
+    h[r].x = g->row_x[r];
+    h[r].padw = g->row_padw[r];
+    h[r].inv_padw = g->row_inv_padw[r];
+    h[r].half = (float)(g->row_npads[r] / 2);   // exact in binary32
+  }
+  cudaError_t e = cudaMalloc(&ctx->d_rows, sizeof(RowGeo) * g->n_rows);
+  if (e == cudaSuccess) e = cudaMemcpy(ctx->d_rows, h, sizeof(RowGeo) * g->n_rows, cudaMemcpyHostToDevice);
+  free(h);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(CHUNK_WINDOW * 4 + (size_t)g->n_sectors_out * g->n_rows * 8));
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    if (ctx->d_rows) cudaFree(ctx->d_rows);
+    delete ctx;
+    return TMD_ERR_CUDA;
+  }
+  DevGeo& G = ctx->geo;
+  G.n_az = g->n_az; G.n_sides = g->n_sides; G.n_sectors_out = g->n_sectors_out; G.n_rows = g->n_rows;
+  G.n_bins = g->n_sectors_out * g->n_rows;
+  G.cos_a = g->cos_a; G.sin_a = g->sin_a;
+  // KB = bz * 0.00299792458f; QK = 0.0625f * KB: two single binary32 multiplications (volatile: no folding into one)
+  volatile float kb = f->bz_tesla * 0.00299792458f;
+  volatile float qk = 0.0625f * kb;
+  G.qk = qk;
+  G.rows = ctx->d_rows;
+  *out_ctx = ctx;
+  return TMD_OK;
+}
+
+int tmd_workspace_bytes(const tmd_ctx* ctx, uint32_t n_tracks, uint64_t n_att, uint64_t n_unatt, size_t* out_bytes) {
+  if (!ctx || !out_bytes) return TMD_ERR_ARG;
+  if (n_att + n_unatt >= (1ull << 32) || n_att < n_tracks) return TMD_ERR_ARG;
+  *out_bytes = layout(ctx->geo.n_bins, n_tracks, n_att).total;
+  return TMD_OK;
+}
+
+int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
+  int rc = check_args(ctx, in, out, true);
+  if (rc != TMD_OK) return rc;
+  const DevGeo& G = ctx->geo;
+  const uint32_t n_trk = in->n_tracks, n_bins = G.n_bins;
+  const uint32_t n_att = (uint32_t)in->n_attached, n_un = (uint32_t)in->n_unattached;
+  const Workspace W = layout(n_bins, n_trk, n_att);
+  if (!out->workspace || out->workspace_bytes < W.total) return TMD_ERR_WORKSPACE;
+  if (misaligned(out->workspace, ALIGN)) return TMD_ERR_ALIGN;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)out->workspace;
+  uint32_t* d_err = (uint32_t*)(ws + W.o_err);
+  uint32_t* d_tile = (uint32_t*)(ws + W.o_tile_sum);
+  uint32_t* d_off = (uint32_t*)(ws + W.o_off);
+  uint32_t* d_cfirst = (uint32_t*)(ws + W.o_chunk_first);
+  uint32_t* d_attcnt = (uint32_t*)(ws + W.o_att_cnt);
+  uint32_t* d_ustart = (uint32_t*)(ws + W.o_u_start);
+  uint32_t* d_gsum = (uint32_t*)(ws + W.o_gsum);
+  uint16_t* d_hist = (uint16_t*)(ws + W.o_hist);
+  uint32_t* d_rel = (uint32_t*)(ws + W.o_rel);
+  uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
+  const bool validate = (flags & TMD_VALIDATE) != 0;
+  ctx->launches = 0;
+  if (cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+
+  if (n_trk > 0) {  // A1: track offsets + chunk table
+    k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile);
+    TMD_LAUNCH_CHECK();
+    k_scan_tile_sums<<<1, 1024, 0, st>>>(d_tile, W.n_tiles);
+    TMD_LAUNCH_CHECK();
+    k_track_offsets<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile, W.n_tiles, d_off);
+    TMD_LAUNCH_CHECK();
+  }
+  if (validate) {
+    k_validate<<<148, 256, 0, st>>>(G, *in, d_off, d_err);
+    TMD_LAUNCH_CHECK();
+    uint32_t h_err[ERR_WORDS];
+    if (cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+    if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;
+  }
+  if (n_trk > 0) {
+    k_chunk_table<<<(n_trk + 1 + 255) / 256, 256, 0, st>>>(d_off, n_trk, d_cfirst, W.n_chunks);
+    TMD_LAUNCH_CHECK();
+    // A3: walk + per-chunk histogram + ranks
+    RankArgs R;
+    R.off = d_off; R.chunk_first = d_cfirst; R.trk_row0 = in->trk_row0; R.trk_sec0 = in->trk_sec0;
+    R.a_rowdiff = in->a_rowdiff; R.a_secleg = in->a_secleg; R.hist = d_hist; R.rank16 = d_rank;
+    R.n_chunks = W.n_chunks; R.n_tracks = n_trk; R.n_attached = n_att;
+    const size_t rank_smem = CHUNK_WINDOW * 4 + (size_t)n_bins * 8;
+    k_rank<<<W.n_chunks, RANK_THREADS, rank_smem, st>>>(G, R);
+    TMD_LAUNCH_CHECK();
+    // A4: column scan over chunks
+    dim3 cg((n_bins + 255) / 256, W.n_groups);
+    k_col_group_sums<<<cg, 256, 0, st>>>(d_hist, W.n_chunks, n_bins, d_gsum);
+    TMD_LAUNCH_CHECK();
+    k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, st>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
+    TMD_LAUNCH_CHECK();
+  } else {
+    if (cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+  }
+  k_bin_offsets<<<1, 1024, 0, st>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
+  TMD_LAUNCH_CHECK();
+  if (n_trk > 0) {
+    dim3 cg((n_bins + 255) / 256, W.n_groups);
+    k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
+    TMD_LAUNCH_CHECK();
+    // A5 + A6
+    DecodeArgs D;
+    D.off = d_off; D.rel = d_rel; D.rank16 = d_rank; D.in = *in; D.clusters = (uint4*)out->clusters;
+    D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
+    D.n_clusters_total = n_att + n_un;
+    k_decode_attached<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, sizeof(RowGeo) * G.n_rows, st>>>(G, D);
+    TMD_LAUNCH_CHECK();
+  }
+  if (n_un > 0) {  // A7
+    UnattachedArgs U;
+    U.in = *in; U.u_start = d_ustart; U.bin_offset = out->bin_offset; U.att_cnt = d_attcnt;
+    U.clusters = (uint4*)out->clusters; U.n_clusters_total = n_att + n_un;
+    k_unattached<<<n_bins, UNATT_THREADS, 0, st>>>(G, U);
+    TMD_LAUNCH_CHECK();
+  }
+  if (validate) {
+    uint32_t h_err[ERR_WORDS];
+    if (cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+    if (h_err[ERR_TRACK_FIELD] || h_err[ERR_SECTOR_OUT]) return TMD_ERR_CORRUPT;
+  }
+  return TMD_OK;
+}
+
+int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
+  int rc = check_args(ctx, in, out, false);
+  if (rc != TMD_OK) return rc;
+  const uint32_t n_bins = ctx->geo.n_bins;
+  const size_t n_trk = in->n_tracks, n_att = in->n_attached, n_res = n_att - n_trk, n_un = in->n_unattached;
+  const Workspace W = layout(n_bins, in->n_tracks, n_att);
+  // arena: inputs, outputs, workspace
+  struct Seg { const void* src; size_t bytes; size_t at; };
+  Seg segs[] = {
+      {in->trk_ncl, n_trk * 2, 0},   {in->trk_qpt, n_trk, 0},      {in->trk_row0, n_trk, 0},    {in->trk_sec0, n_trk, 0},
+      {in->trk_pad0, n_trk * 2, 0},  {in->trk_time0, n_trk * 4, 0},
+      {in->a_qtot, n_att * 2, 0},    {in->a_qmax, n_att * 2, 0},   {in->a_flags, n_att, 0},     {in->a_sigpad, n_att, 0},
+      {in->a_sigtime, n_att, 0},
+      {in->a_rowdiff, n_res, 0},     {in->a_secleg, n_res, 0},     {in->a_padres, n_res * 2, 0}, {in->a_timeres, n_res * 4, 0},
+      {in->u_qtot, n_un * 2, 0},     {in->u_qmax, n_un * 2, 0},    {in->u_flags, n_un, 0},      {in->u_sigpad, n_un, 0},
+      {in->u_sigtime, n_un, 0},      {in->u_paddiff, n_un * 2, 0}, {in->u_timediff, n_un * 4, 0},
+      {in->u_bin_count, (size_t)n_bins * 4, 0}};
+  size_t o = 0;
+  for (Seg& s : segs) { s.at = o; o += align_up(s.bytes); }
+  const size_t o_clusters = o; o += align_up((n_att + n_un) * 16);
+  const size_t o_binoff = o;   o += align_up(((size_t)n_bins + 1) * 4);
+  const size_t o_probe = o;    o += align_up(out->probe_state ? n_trk * 24 : 0);
+  const size_t o_ws = o;       o += W.total;
+  if (o > ctx->arena_bytes) {
+    if (ctx->arena) cudaFree(ctx->arena);
+    ctx->arena = nullptr; ctx->arena_bytes = 0;
+    if (cudaMalloc(&ctx->arena, o) != cudaSuccess) { cudaGetLastError(); return TMD_ERR_CUDA; }
+    ctx->arena_bytes = o;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* a = (unsigned char*)ctx->arena;
+  for (const Seg& s : segs)
+    if (s.bytes && cudaMemcpyAsync(a + s.at, s.src, s.bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TMD_ERR_CUDA;
+  tmd_compressed d = *in;
+  const void** dst[] = {(const void**)&d.trk_ncl, (const void**)&d.trk_qpt, (const void**)&d.trk_row0, (const void**)&d.trk_sec0,
+                        (const void**)&d.trk_pad0, (const void**)&d.trk_time0, (const void**)&d.a_qtot, (const void**)&d.a_qmax,
+                        (const void**)&d.a_flags, (const void**)&d.a_sigpad, (const void**)&d.a_sigtime, (const void**)&d.a_rowdiff,
+                        (const void**)&d.a_secleg, (const void**)&d.a_padres, (const void**)&d.a_timeres, (const void**)&d.u_qtot,
+                        (const void**)&d.u_qmax, (const void**)&d.u_flags, (const void**)&d.u_sigpad, (const void**)&d.u_sigtime,
+                        (const void**)&d.u_paddiff, (const void**)&d.u_timediff, (const void**)&d.u_bin_count};
+  for (size_t i = 0; i < sizeof(segs) / sizeof(segs[0]); ++i) *dst[i] = a + segs[i].at;
+  tmd_output dout = *out;
+  dout.clusters = (tmd_cluster*)(a + o_clusters);
+  dout.bin_offset = (uint32_t*)(a + o_binoff);
+  dout.probe_state = out->probe_state ? (uint32_t*)(a + o_probe) : nullptr;
+  dout.workspace = a + o_ws;
+  dout.workspace_bytes = W.total;
+  rc = tmd_decode(ctx, &d, &dout, flags, cuda_stream);
+  if (rc != TMD_OK) return rc;
+  if ((n_att + n_un) && cudaMemcpyAsync(out->clusters, dout.clusters, (n_att + n_un) * 16, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    return TMD_ERR_CUDA;
+  if (cudaMemcpyAsync(out->bin_offset, dout.bin_offset, ((size_t)n_bins + 1) * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    return TMD_ERR_CUDA;
+  if (out->probe_state && n_trk &&
+      cudaMemcpyAsync(out->probe_state, dout.probe_state, n_trk * 24, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    return TMD_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+  return TMD_OK;
+}
+
+int tmd_destroy(tmd_ctx* ctx) {
+  if (!ctx) return TMD_OK;
+  if (ctx->arena) cudaFree(ctx->arena);
+  if (ctx->d_rows) cudaFree(ctx->d_rows);
+  delete ctx;
+  return TMD_OK;
+}
+
+const char* tmd_status_string(int status) {
+  switch (status) {
+    case TMD_OK: return "ok";
+    case TMD_ERR_ARG: return "bad argument";
+    case TMD_ERR_ALIGN: return "misaligned pointer";
+    case TMD_ERR_WORKSPACE: return "workspace missing or too small";
+    case TMD_ERR_CUDA: return "CUDA runtime error";
+    case TMD_ERR_CORRUPT: return "inconsistent compressed input";
+    default: return "unknown status";
+  }
+}
+
+int tmd_last_launch_count(const tmd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,63 @@
+// tmd_common.cuh -- shared definitions of the sm_100a track-model decoder kernels.
+//
+// Model = SURVEY.md §8(c) C1-C5 (readings listed in DESIGN.md §3); paper passages: PAPER.md L68, L70.
+// No code is shared with oracle/ (own structs, constants and helpers).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tmd.h"
+
+namespace tmd {
+
+// A "chunk" is the set of tracks whose first cluster's global attached index g = off[t] falls in one window of
+// 2^CHUNK_SHIFT clusters.  Chunks are the unit of the deterministic scatter: per-chunk histograms over
+// bins, a column scan over chunks, and ranks inside the chunk.
+constexpr int CHUNK_SHIFT = 15;
+constexpr uint32_t CHUNK_WINDOW = 1u << CHUNK_SHIFT;
+constexpr uint32_t RANK_CAP = 36864;    // clusters of a chunk that the shared-memory rank path can hold
+constexpr uint32_t MAX_BINS = 8192;     // n_sectors_out * n_rows
+constexpr uint32_t COL_GROUP = 64;      // chunks per group in the column scan
+constexpr uint16_t BIN_INVALID = 0xFFFFu;
+
+struct RowGeo {   // one LDS.128 per step
+  float x, padw, inv_padw, half;
+};
+
+struct DevGeo {
+  uint32_t n_az, n_sides, n_sectors_out, n_rows, n_bins;
+  float cos_a, sin_a;
+  float qk;             // fmul(0.0625f, fmul(bz_tesla, 0.00299792458f))
+  const RowGeo* rows;   // DEVICE [n_rows]
+};
+
+// error word indices in the workspace (TMD_VALIDATE)
+enum { ERR_TRACK_FIELD = 0, ERR_SECTOR_OUT = 1, ERR_WORDS = 4 };
+
+// ---- the integer part of one step: leg / row / sector bookkeeping (C3-3, C3-4, C3-5 without the rotation) ----------
+struct WalkState {
+  uint32_t row, az, side;
+  int dir;
+};
+
+__device__ __forceinline__ uint32_t reduce_mod(uint32_t v, uint32_t m) {  // v < 256, m >= 1 (reading 19)
+  while (v >= m) v -= m;
+  return v;
+}
+
+// returns the reduced sector step d (0 = same sector); updates row / az / dir
+__device__ __forceinline__ uint32_t walk_step(WalkState& w, uint32_t rowdiff, uint32_t secleg, uint32_t n_rows, uint32_t n_az) {
+  if (secleg & 0x80u) w.dir = -w.dir;
+  uint32_t rd = reduce_mod(rowdiff, n_rows);
+  uint32_t r = w.row + (w.dir > 0 ? rd : n_rows - rd);
+  w.row = r >= n_rows ? r - n_rows : r;
+  uint32_t d = reduce_mod(secleg & 0x3Fu, n_az);
+  uint32_t a = w.az + d;
+  w.az = a >= n_az ? a - n_az : a;
+  return d;
+}
+
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
+
+}  // namespace tmd

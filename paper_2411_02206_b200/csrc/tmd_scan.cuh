@@ -1,0 +1,189 @@
+// tmd_scan.cuh -- prefix sums of the decoder: track offsets (A1), chunk table, column scan over chunks and bin
+// offsets (A4).  Integer only.
+#pragma once
+
+#include "tmd_common.cuh"
+
+namespace tmd {
+
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t n = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane_id() >= (uint32_t)o) v += n;
+  }
+  return v;
+}
+
+// Exclusive scan of one value per thread over the block; returns the exclusive prefix, *total = block sum.
+// `ws` = 33 words of shared memory.  Contains __syncthreads (all threads must call).
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, uint32_t* total) {
+  const uint32_t lane = lane_id(), wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  uint32_t inc = warp_incl_scan(v);
+  __syncthreads();  // protect ws from a previous call
+  if (lane == 31) ws[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t s = lane < nw ? ws[lane] : 0;
+    uint32_t si = warp_incl_scan(s);
+    ws[lane] = si - s;
+    if (lane == 31) ws[32] = si;
+  }
+  __syncthreads();
+  *total = ws[32];
+  return ws[wid] + inc - v;
+}
+
+// ---- A1: off[t] = exclusive prefix sum of trk_ncl (PAPER.md L70 precomputes these indices on the CPU) --------------
+constexpr int SCAN_THREADS = 512;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_track_tile_sums(const uint16_t* __restrict__ trk_ncl, uint32_t n_tracks,
+                                                                 uint32_t* __restrict__ tile_sum) {
+  __shared__ uint32_t ws[33];
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t s = 0;
+  if (base + SCAN_ITEMS <= n_tracks) {
+    uint4 v = *reinterpret_cast<const uint4*>(trk_ncl + base);  // 8 x u16, 16-byte aligned
+    s = (v.x & 0xFFFFu) + (v.x >> 16) + (v.y & 0xFFFFu) + (v.y >> 16) + (v.z & 0xFFFFu) + (v.z >> 16) + (v.w & 0xFFFFu) + (v.w >> 16);
+  } else {
+    for (uint32_t i = base; i < n_tracks && i < base + SCAN_ITEMS; ++i) s += trk_ncl[i];
+  }
+  uint32_t total;
+  block_excl_scan(s, ws, &total);
+  if (threadIdx.x == 0) tile_sum[blockIdx.x] = total;
+}
+
+// single block: exclusive scan of tile_sum in place; tile_sum[n_tiles] = grand total
+__global__ void __launch_bounds__(1024) k_scan_tile_sums(uint32_t* __restrict__ tile_sum, uint32_t n_tiles) {
+  __shared__ uint32_t ws[33];
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n_tiles; base += blockDim.x) {
+    uint32_t i = base + threadIdx.x;
+    uint32_t v = i < n_tiles ? tile_sum[i] : 0, total;
+    uint32_t ex = block_excl_scan(v, ws, &total);
+    if (i < n_tiles) tile_sum[i] = carry + ex;
+    carry += total;
+  }
+  if (threadIdx.x == 0) tile_sum[n_tiles] = carry;
+}
+
+// off[t] for every track; off[n_tracks] = total
+__global__ void __launch_bounds__(SCAN_THREADS) k_track_offsets(const uint16_t* __restrict__ trk_ncl, uint32_t n_tracks,
+                                                               const uint32_t* __restrict__ tile_sum, uint32_t n_tiles,
+                                                               uint32_t* __restrict__ off) {
+  __shared__ uint32_t ws[33];
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    v[k] = (base + k < n_tracks) ? trk_ncl[base + k] : 0;
+    s += v[k];
+  }
+  uint32_t total;
+  uint32_t run = tile_sum[blockIdx.x] + block_excl_scan(s, ws, &total);
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    if (base + k < n_tracks) off[base + k] = run;
+    run += v[k];
+  }
+  if (blockIdx.x == n_tiles - 1 && threadIdx.x == 0) off[n_tracks] = tile_sum[n_tiles];
+}
+
+// Chunk table: chunk c = the tracks t with (off[t] >> CHUNK_SHIFT) == c = [chunk_first[c], chunk_first[c+1]).
+// chunk_first[c] = first track with off[t] >= c << CHUNK_SHIFT; off is strictly increasing (trk_ncl >= 1), so track t
+// is that first track for every c with off[t-1] < c*W <= off[t].  One thread per t in [0, n_tracks].
+__global__ void k_chunk_table(const uint32_t* __restrict__ off, uint32_t n_tracks, uint32_t* __restrict__ chunk_first,
+                              uint32_t n_chunks) {
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t > n_tracks) return;
+  const uint32_t c_lo = (t == 0) ? 0 : (off[t - 1] >> CHUNK_SHIFT) + 1;
+  uint32_t c_hi = (t == n_tracks) ? n_chunks : (off[t] >> CHUNK_SHIFT);
+  if (c_hi > n_chunks) c_hi = n_chunks;  // malformed counts must not write out of bounds
+  for (uint32_t c = c_lo; c <= c_hi; ++c) chunk_first[c] = t;
+}
+
+// ---- A4 part 1: column sums over groups of chunks ---------------------------------------------------------------------
+// hist[c][b] (u16) = attached clusters of chunk c in bin b.   gsum[grp][b] = sum over the group's chunks.
+__global__ void __launch_bounds__(256) k_col_group_sums(const uint16_t* __restrict__ hist, uint32_t n_chunks, uint32_t n_bins,
+                                                        uint32_t* __restrict__ gsum) {
+  const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x, grp = blockIdx.y;
+  if (b >= n_bins) return;
+  const uint32_t c0 = grp * COL_GROUP, c1 = min(c0 + COL_GROUP, n_chunks);
+  uint32_t s = 0;
+#pragma unroll 8
+  for (uint32_t c = c0; c < c1; ++c) s += hist[(size_t)c * n_bins + b];
+  gsum[(size_t)grp * n_bins + b] = s;
+}
+
+// per bin: exclusive scan of gsum over groups (in place), att_cnt[b] = total
+__global__ void __launch_bounds__(256) k_col_group_scan(uint32_t* __restrict__ gsum, uint32_t n_groups, uint32_t n_bins,
+                                                        uint32_t* __restrict__ att_cnt) {
+  const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= n_bins) return;
+  uint32_t run = 0;
+  uint32_t g = 0;
+  for (; g + 8 <= n_groups; g += 8) {
+    uint32_t v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = gsum[(size_t)(g + k) * n_bins + b];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      gsum[(size_t)(g + k) * n_bins + b] = run;
+      run += v[k];
+    }
+  }
+  for (; g < n_groups; ++g) {
+    uint32_t v = gsum[(size_t)g * n_bins + b];
+    gsum[(size_t)g * n_bins + b] = run;
+    run += v;
+  }
+  att_cnt[b] = run;
+}
+
+// single block: bin_offset[b] = exclusive scan of att_cnt[b] + u_cnt[b]; u_start[b] = exclusive scan of u_cnt[b]
+// (C5: a bin holds its attached clusters first, then its unattached ones).  totals[0] = sum u_cnt.
+__global__ void __launch_bounds__(1024) k_bin_offsets(const uint32_t* __restrict__ att_cnt, const uint32_t* __restrict__ u_cnt,
+                                                      uint32_t n_bins, uint32_t* __restrict__ bin_offset,
+                                                      uint32_t* __restrict__ u_start) {
+  __shared__ uint32_t ws[33];
+  const uint32_t per = (n_bins + blockDim.x - 1) / blockDim.x;
+  const uint32_t b0 = threadIdx.x * per, b1 = min(b0 + per, n_bins);
+  uint32_t sa = 0, su = 0;
+  for (uint32_t b = b0; b < b1; ++b) {
+    su += u_cnt[b];
+    sa += att_cnt[b] + u_cnt[b];
+  }
+  uint32_t ta, tu;
+  uint32_t ea = block_excl_scan(sa, ws, &ta);
+  uint32_t eu = block_excl_scan(su, ws, &tu);
+  for (uint32_t b = b0; b < b1; ++b) {
+    bin_offset[b] = ea;
+    u_start[b] = eu;
+    eu += u_cnt[b];
+    ea += att_cnt[b] + u_cnt[b];
+  }
+  if (threadIdx.x == 0) {
+    bin_offset[n_bins] = ta;
+    u_start[n_bins] = tu;
+  }
+}
+
+// ---- A4 part 2: rel[c][b] = bin_offset[b] + attached clusters of bin b in chunks < c ---------------------------------
+__global__ void __launch_bounds__(256) k_col_apply(const uint16_t* __restrict__ hist, const uint32_t* __restrict__ gsum,
+                                                   const uint32_t* __restrict__ bin_offset, uint32_t n_chunks, uint32_t n_bins,
+                                                   uint32_t* __restrict__ rel) {
+  const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x, grp = blockIdx.y;
+  if (b >= n_bins) return;
+  const uint32_t c0 = grp * COL_GROUP, c1 = min(c0 + COL_GROUP, n_chunks);
+  uint32_t run = bin_offset[b] + gsum[(size_t)grp * n_bins + b];
+#pragma unroll 8
+  for (uint32_t c = c0; c < c1; ++c) {
+    const uint32_t h = hist[(size_t)c * n_bins + b];
+    rel[(size_t)c * n_bins + b] = run;
+    run += h;
+  }
+}
+
+}  // namespace tmd

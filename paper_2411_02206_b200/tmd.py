@@ -1,0 +1,150 @@
+"""ctypes binding of libtmd.so -- same names as include/tmd.h, argument marshalling only.
+
+Every step of the path (offsets scan, geometry walk + ranks, column scan, track-model decode, scatter, unattached
+prefix sums) runs in the CUDA kernels of csrc/.  PyTorch supplies device memory and streams, nothing else.
+PAPER.md L68/L70 define the operation; include/tmd.h states layout, ownership and error behaviour.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT = 0, -1, -2, -3, -4, -5
+TMD_VALIDATE = 1
+PROBE_FINAL = 0xFFFFFFFF
+
+# (field name, numpy dtype) in the order of struct tmd_compressed
+COMPRESSED_ARRAYS = (
+    ("trk_ncl", "<u2"), ("trk_qpt", "i1"), ("trk_row0", "u1"), ("trk_sec0", "u1"), ("trk_pad0", "<u2"), ("trk_time0", "<u4"),
+    ("a_qtot", "<u2"), ("a_qmax", "<u2"), ("a_flags", "u1"), ("a_sigpad", "u1"), ("a_sigtime", "u1"),
+    ("a_rowdiff", "u1"), ("a_secleg", "u1"), ("a_padres", "<u2"), ("a_timeres", "<u4"),
+    ("u_qtot", "<u2"), ("u_qmax", "<u2"), ("u_flags", "u1"), ("u_sigpad", "u1"), ("u_sigtime", "u1"),
+    ("u_paddiff", "<u2"), ("u_timediff", "<u4"), ("u_bin_count", "<u4"),
+)
+
+
+class tmd_geometry(C.Structure):
+    _fields_ = [("n_az", C.c_uint32), ("n_sides", C.c_uint32), ("n_sectors_out", C.c_uint32), ("n_rows", C.c_uint32),
+                ("cos_a", C.c_float), ("sin_a", C.c_float),
+                ("row_x", C.c_void_p), ("row_padw", C.c_void_p), ("row_inv_padw", C.c_void_p), ("row_npads", C.c_void_p)]
+
+
+class tmd_field(C.Structure):
+    _fields_ = [("bz_tesla", C.c_float)]
+
+
+class tmd_compressed(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint32), ("n_attached", C.c_uint64), ("n_unattached", C.c_uint64)] + \
+               [(k, C.c_void_p) for k, _ in COMPRESSED_ARRAYS]
+
+
+class tmd_output(C.Structure):
+    _fields_ = [("clusters", C.c_void_p), ("bin_offset", C.c_void_p), ("probe_state", C.c_void_p),
+                ("probe_step", C.c_uint32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load (building first if the sources are newer) libtmd.so.  Raises if that is impossible: no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        L.tmd_create.argtypes = [C.POINTER(tmd_geometry), C.POINTER(tmd_field), C.POINTER(C.c_void_p)]
+        L.tmd_workspace_bytes.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_uint64, C.POINTER(C.c_size_t)]
+        L.tmd_decode.argtypes = [C.c_void_p, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_void_p]
+        L.tmd_decode_host.argtypes = L.tmd_decode.argtypes
+        L.tmd_destroy.argtypes = [C.c_void_p]
+        L.tmd_status_string.argtypes = [C.c_int]
+        L.tmd_status_string.restype = C.c_char_p
+        L.tmd_last_launch_count.argtypes = [C.c_void_p]
+        for f in (L.tmd_create, L.tmd_workspace_bytes, L.tmd_decode, L.tmd_decode_host, L.tmd_destroy, L.tmd_last_launch_count):
+            f.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+class TmdError(RuntimeError):
+    def __init__(self, status: int):
+        self.status = status
+        super().__init__(f"tmd status {status}: {tmd_status_string(status)}")
+
+
+def tmd_status_string(status: int) -> str:
+    return lib().tmd_status_string(status).decode()
+
+
+def _check(rc: int) -> None:
+    if rc != TMD_OK:
+        raise TmdError(rc)
+
+
+def _ptr(a) -> int | None:
+    """Address of a torch tensor (device or host) or numpy array; None for absent / empty arrays."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data if a.size else None
+    assert a.is_contiguous()
+    return a.data_ptr() if a.numel() else None
+
+
+def tmd_create(geo, bz_tesla: float) -> int:
+    """tmd_create(geometry, field) -> opaque context handle.  `geo` = tmd_inputs.geometry.Geometry (tables as inputs)."""
+    keep = [np.ascontiguousarray(geo.row_x, np.float32), np.ascontiguousarray(geo.row_padw, np.float32),
+            np.ascontiguousarray(geo.row_inv_padw, np.float32), np.ascontiguousarray(geo.row_npads, np.uint16)]
+    g = tmd_geometry(geo.n_az, geo.n_sides, geo.n_sectors_out, geo.n_rows, float(geo.cos_a), float(geo.sin_a),
+                     *(k.ctypes.data for k in keep))
+    f = tmd_field(float(np.float32(bz_tesla)))
+    ctx = C.c_void_p()
+    _check(lib().tmd_create(C.byref(g), C.byref(f), C.byref(ctx)))
+    return ctx.value
+
+
+def tmd_destroy(ctx: int) -> None:
+    _check(lib().tmd_destroy(ctx))
+
+
+def tmd_workspace_bytes(ctx: int, n_tracks: int, n_attached: int, n_unattached: int) -> int:
+    out = C.c_size_t()
+    _check(lib().tmd_workspace_bytes(ctx, n_tracks, n_attached, n_unattached, C.byref(out)))
+    return out.value
+
+
+def tmd_last_launch_count(ctx: int) -> int:
+    return lib().tmd_last_launch_count(ctx)
+
+
+def make_compressed(arrays: dict) -> tmd_compressed:
+    """struct tmd_compressed from a dict name -> tensor/ndarray (all on the device, or all on the host)."""
+    n_trk = int(arrays["trk_ncl"].shape[0])
+    n_att = int(arrays["a_qtot"].shape[0])
+    n_un = int(arrays["u_qtot"].shape[0])
+    c = tmd_compressed(n_trk, n_att, n_un)
+    for k, _ in COMPRESSED_ARRAYS:
+        setattr(c, k, _ptr(arrays[k]))
+    return c
+
+
+def make_output(clusters, bin_offset, workspace=None, probe_state=None, probe_step: int = PROBE_FINAL) -> tmd_output:
+    ws_bytes = 0 if workspace is None else int(workspace.numel() * workspace.element_size())
+    return tmd_output(_ptr(clusters), _ptr(bin_offset), _ptr(probe_state), probe_step, _ptr(workspace), ws_bytes)
+
+
+def tmd_decode(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, stream: int = 0) -> None:
+    """Enqueue the decode of one time frame on CUDA stream handle `stream` (DEVICE pointers)."""
+    _check(lib().tmd_decode(ctx, C.byref(comp), C.byref(out), flags, stream))
+
+
+def tmd_decode_host(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, stream: int = 0) -> None:
+    """End-to-end decode with HOST pointers (copies in, decodes, copies out, synchronises)."""
+    _check(lib().tmd_decode_host(ctx, C.byref(comp), C.byref(out), flags, stream))

@@ -1,0 +1,156 @@
+"""`-m gpu` parity: the CUDA library (through its C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): bit-exact on every integer cluster field in canonical order, bin offsets equal, and the
+fp32 track-state probes equal to the oracle's at 0 ULP (no FMA contraction on either side).  Inputs are seeded and
+synthetic: helix events encoded by the oracle encoder (configs c0, c1 full size, c2/c4-shaped), adversarial random bytes
+and degenerate cases.
+"""
+import numpy as np
+import pytest
+
+from oracle import tmd_oracle as O
+from tmd_inputs import build_geometry, physical as ph
+from tmd_inputs.adversarial import degenerate_same_bin, random_compressed
+from tmd_inputs.layout import Compressed
+
+from gpu_util import first_mismatch, gpu_decode
+
+pytestmark = pytest.mark.gpu
+BZ = 0.5
+
+PHYS = {
+    "c0": (lambda: ph.config0(), 2),
+    "c1": (lambda: ph.config1(), 36),
+    "c2_like": (lambda: ph.config2_like(6000, 90_000), 36),
+    "c4_like": (lambda: ph.config4_like(40_000, 100_000), 36),
+}
+
+
+def assert_same(got, want):
+    g_cl, g_bo, g_pr = got
+    w_cl, w_bo, w_pr = want
+    assert np.array_equal(g_bo, w_bo), "bin_offset: " + first_mismatch(g_bo, w_bo)
+    for f in w_cl.dtype.names:
+        assert np.array_equal(g_cl[f], w_cl[f]), f"{f}: " + first_mismatch(g_cl[f], w_cl[f])
+    assert g_cl.tobytes() == w_cl.tobytes()
+    if w_pr is not None:
+        nan = np.isnan(w_pr.view(np.float32))            # NaN payloads are not compared (reading 15)
+        assert np.array_equal(np.isnan(g_pr.view(np.float32)), nan)
+        ulp = np.abs(g_pr.astype(np.int64) - w_pr.astype(np.int64))[~nan]
+        assert ulp.max(initial=0) == 0, f"probe state deviates by up to {ulp.max()} ULP in {np.count_nonzero(ulp)} values"
+
+
+@pytest.fixture(scope="module", params=list(PHYS))
+def phys_case(request):
+    mk, nsec = PHYS[request.param]
+    geo = build_geometry(nsec)
+    ev = ph.generate_event(mk(), geo)
+    comp = O.encode(geo, BZ, ev.trk_ncl, ev.trk_qptf, ev.att, ev.leg, ev.un)
+    return request.param, geo, ev, comp
+
+
+def test_physical_events_match_oracle(phys_case):
+    name, geo, ev, comp = phys_case
+    assert_same(gpu_decode(geo, BZ, comp, probe_step=0xFFFFFFFF), O.decode(geo, BZ, comp, probe_step=0xFFFFFFFF))
+
+
+def test_physical_events_round_trip(phys_case):
+    # decode(encode(x)) == canonical(x): the GPU decoder restores the generator's clusters
+    name, geo, ev, comp = phys_case
+    cl, bo, _ = gpu_decode(geo, BZ, comp)
+    want, want_bo = ph.canonical(ev, geo)
+    assert np.array_equal(bo, want_bo) and cl.tobytes() == want.tobytes()
+
+
+@pytest.mark.parametrize("step", [0, 1, 7, "half"])
+def test_probes_at_intermediate_steps(phys_case, step):
+    name, geo, ev, comp = phys_case
+    if name not in ("c0", "c4_like"):
+        pytest.skip("probe sweep on two cases")
+    s = int(np.median(comp.trk_ncl)) // 2 if step == "half" else step
+    assert_same(gpu_decode(geo, BZ, comp, probe_step=s), O.decode(geo, BZ, comp, probe_step=s))
+
+
+def test_host_entry_point_matches(phys_case):
+    name, geo, ev, comp = phys_case
+    if name != "c0":
+        pytest.skip("one case")
+    assert_same(gpu_decode(geo, BZ, comp, probe_step=3, via_host=True), O.decode(geo, BZ, comp, probe_step=3))
+
+
+@pytest.mark.parametrize("seed,n_tracks,n_un,max_ncl", [(1, 300, 4000, 40), (2, 1, 0, 40), (3, 50, 0, 40), (4, 0, 100, 40),
+                                                       (5, 20_000, 150_000, 200), (6, 3000, 0, 1000)])
+def test_adversarial_random_bytes(seed, n_tracks, n_un, max_ncl):
+    geo = build_geometry(36)
+    c = random_compressed(geo, n_tracks, n_un, seed, max_ncl=max_ncl)
+    assert_same(gpu_decode(geo, BZ, c, probe_step=0xFFFFFFFF), O.decode(geo, BZ, c, probe_step=0xFFFFFFFF))
+
+
+def test_empty_and_one_sided_inputs():
+    geo = build_geometry(36)
+    c = Compressed.empty(0, 0, 0, geo.n_bins)
+    cl, bo, _ = gpu_decode(geo, BZ, c)
+    assert len(cl) == 0 and np.all(bo == 0)
+    c = random_compressed(geo, 0, 0, 11, ncl=np.ones(500, np.uint16))       # only single-cluster tracks: no residuals at all
+    assert_same(gpu_decode(geo, BZ, c), O.decode(geo, BZ, c))
+
+
+def test_tracks_longer_than_a_chunk_window():
+    # trk_ncl up to the format's maximum (65535): tracks straddle several 32768-cluster windows of the rank pass
+    geo = build_geometry(36)
+    ncl = np.array([5, 65535, 1, 40000, 32768, 32767, 3, 152, 65535, 9], np.uint16)
+    c = random_compressed(geo, 0, 1000, 12, ncl=ncl)
+    assert_same(gpu_decode(geo, BZ, c, probe_step=0xFFFFFFFF), O.decode(geo, BZ, c, probe_step=0xFFFFFFFF))
+
+
+def test_degenerate_all_clusters_in_one_bin():
+    geo = build_geometry(36)
+    rng = np.random.default_rng(3)
+    ncl = np.concatenate((rng.integers(1, 300, 400), [20000, 1, 1, 9000])).astype(np.uint16)
+    c = degenerate_same_bin(geo, ncl, 13, n_un=500)
+    assert_same(gpu_decode(geo, BZ, c), O.decode(geo, BZ, c))
+
+
+def test_unattached_skewed_bins():
+    geo = build_geometry(36)
+    rng = np.random.default_rng(21)
+    counts = rng.poisson(2.0, geo.n_bins).astype(np.uint32)
+    counts[17] = 300_000           # one bin much larger than a tile
+    counts[18] = 1
+    counts[geo.n_bins - 1] = 5000
+    n = int(counts.sum())
+    c = random_compressed(geo, 10, 0, 22)
+    u = Compressed.empty(c.n_tracks, c.n_attached, n, geo.n_bins)
+    for k in ("trk_ncl", "trk_qpt", "trk_row0", "trk_sec0", "trk_pad0", "trk_time0", "a_qtot", "a_qmax", "a_flags", "a_sigpad",
+              "a_sigtime", "a_rowdiff", "a_secleg", "a_padres", "a_timeres"):
+        getattr(u, k)[:] = getattr(c, k)
+    u.u_bin_count[:] = counts
+    u.u_paddiff[:] = rng.integers(0, 65536, n); u.u_timediff[:] = rng.integers(0, 2 ** 32, n)
+    u.u_qtot[:] = rng.integers(0, 65536, n); u.u_qmax[:] = rng.integers(0, 65536, n)
+    u.u_flags[:] = rng.integers(0, 256, n); u.u_sigpad[:] = rng.integers(0, 256, n); u.u_sigtime[:] = rng.integers(0, 256, n)
+    assert_same(gpu_decode(geo, BZ, u), O.decode(geo, BZ, u))
+
+
+def test_validate_flag_reports_corrupt_counts():
+    from paper_2411_02206_b200 import tmd as T
+    geo = build_geometry(36)
+    c = random_compressed(geo, 100, 100, 31)
+    assert_same(gpu_decode(geo, BZ, c, flags=T.TMD_VALIDATE), O.decode(geo, BZ, c))
+    bad = random_compressed(geo, 100, 100, 31)
+    bad.u_bin_count[5] += 1
+    bad.u_bin_count[6] = max(int(bad.u_bin_count[6]), 1) - 1 if bad.u_bin_count[6] > 0 else 0
+    if int(bad.u_bin_count.sum()) != bad.n_unattached:
+        with pytest.raises(T.TmdError) as e:
+            gpu_decode(geo, BZ, bad, flags=T.TMD_VALIDATE)
+        assert e.value.status == T.TMD_ERR_CORRUPT
+    bad = random_compressed(geo, 100, 100, 31)
+    bad.trk_row0[7] = 200
+    with pytest.raises(T.TmdError) as e:
+        gpu_decode(geo, BZ, bad, flags=T.TMD_VALIDATE)
+    assert e.value.status == T.TMD_ERR_CORRUPT
+    # config 0 geometry (2 output sectors): a decoded sector >= 2 is reported (reading 20)
+    geo2 = build_geometry(2)
+    c2 = random_compressed(geo2, 50, 10, 32, n_sectors_in=36)
+    with pytest.raises(T.TmdError) as e:
+        gpu_decode(geo2, BZ, c2, flags=T.TMD_VALIDATE)
+    assert e.value.status == T.TMD_ERR_CORRUPT

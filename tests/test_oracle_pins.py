@@ -15,6 +15,7 @@ import pytest
 from conftest import parse_golden_trace, residual_meta
 from oracle import tmd_oracle as O
 from tmd_inputs import build_geometry, physical as ph
+from tmd_inputs.adversarial import random_compressed
 from tmd_inputs.layout import CLUSTER_DTYPE, Compressed
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "c9_trace.txt")
@@ -234,29 +235,6 @@ def test_unattached_equals_numpy_cumsum(geo36):
 
 
 # ---------------------------------------------------------------------------------------------- assembly (A1, A3-A6, C5)
-def random_compressed(geo, n_tracks, n_un, seed, max_ncl=40):
-    """Adversarial input: valid counts, random bytes in every value array (SURVEY C8 'adversarial')."""
-    rng = np.random.default_rng(seed)
-    ncl = rng.integers(1, max_ncl + 1, n_tracks).astype(np.uint16)
-    n_att = int(ncl.sum())
-    ucnt = rng.multinomial(n_un, np.full(geo.n_bins, 1.0 / geo.n_bins)).astype(np.uint32)
-    c = Compressed.empty(n_tracks, n_att, n_un, geo.n_bins)
-    c.trk_ncl[:] = ncl
-    c.trk_qpt[:] = rng.integers(-128, 128, n_tracks)
-    c.trk_row0[:] = rng.integers(0, geo.n_rows, n_tracks)
-    c.trk_sec0[:] = rng.integers(0, 36, n_tracks)
-    c.trk_pad0[:] = rng.integers(0, 65536, n_tracks)
-    c.trk_time0[:] = rng.integers(0, 2 ** 32, n_tracks)
-    for k in ("a_qtot", "a_qmax", "a_padres", "u_qtot", "u_qmax", "u_paddiff"):
-        getattr(c, k)[:] = rng.integers(0, 65536, len(getattr(c, k)))
-    for k in ("a_flags", "a_sigpad", "a_sigtime", "a_rowdiff", "a_secleg", "u_flags", "u_sigpad", "u_sigtime"):
-        getattr(c, k)[:] = rng.integers(0, 256, len(getattr(c, k)))
-    for k in ("a_timeres", "u_timediff"):
-        getattr(c, k)[:] = rng.integers(0, 2 ** 32, len(getattr(c, k)))
-    c.u_bin_count[:] = ucnt
-    return c
-
-
 def brute_force_decode(geo, c):
     """Per-track decode with slices cut by numpy.cumsum, canonical order by numpy stable argsort."""
     ncl = c.trk_ncl.astype(np.int64)
