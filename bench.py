@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- decoded TPC clusters/s of the track-model decoder on synthetic time frames (BASELINE.json metric).
+
+One "step" = one pass of the whole hot path over one synthetic time frame:
+`tmd_decode` through the C ABI, compressed SoA resident in HBM.  Prints ONE JSON line (see the task contract):
+value = clusters decoded per second over all ranks (device-timed with CUDA events, max over ranks), `e2e` = the same
+through `tmd_decode_host` with pinned HOST buffers (copies inside the timed region), `roofline` for the dominant kernel
+(timed live with CUDA events the library records on the launching stream), `cpu_baseline` = the CPU oracle on a bounded
+sample of the same workload.
+
+Multi-GPU: the path does not shard ("replicas only") -- every rank decodes its own time frame
+(different seed), no collective on the data path; torch.distributed (NCCL) is used for the barrier and the max.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands, single thread) on bounded samples of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+BZ = 0.5
+METRIC = "decoded_tpc_clusters_per_second"
+UNIT = "clusters/s"
+
+
+def algorithmic_bytes_attached(n_trk: int, n_att: int) -> int:
+    """per-track 11 B + copy-through 7 B/cluster + residual streams 8 B/residual in, 16 B/cluster out."""
+    return 11 * n_trk + 7 * n_att + 8 * (n_att - n_trk) + 16 * n_att
+
+
+def algorithmic_bytes_unattached(n_un: int, n_bins: int) -> int:
+    return 13 * n_un + 4 * n_bins + 16 * n_un + 4 * (n_bins + 1)
+
+
+# ------------------------------------------------------------------------------------------------ workload on the device
+def build_workload(name: str, device, seed_offset: int = 0):
+    """Synthetic time frame `name` (tmd_inputs.timeframe.WORKLOADS) as device tensors of the compressed SoA.
+    Attached clusters: helix truth -> the library's own encoder (tmd_encode_attached); unattached: compressed domain."""
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs import build_geometry, timeframe as tf
+
+    geo = build_geometry(36)
+    mk, n_un, single = tf.WORKLOADS[name]
+    cfg = mk()
+    cfg.seed += 1000 * seed_offset
+    truth = tf.generate_truth(cfg, geo, device, batch=2_000_000)
+    n_trk, n_att = truth.n_tracks, truth.n_attached
+    arrays = {"trk_ncl": truth.trk_ncl}
+    spec = dict(T.COMPRESSED_ARRAYS)
+    tdt = {"<u2": torch.int16, "i1": torch.int8, "u1": torch.uint8, "<u4": torch.int32}
+    for k in ("trk_qpt", "trk_row0", "trk_sec0", "trk_pad0", "trk_time0"):
+        arrays[k] = torch.empty(n_trk, dtype=tdt[spec[k]], device=device)
+    for k in ("a_qtot", "a_qmax", "a_flags", "a_sigpad", "a_sigtime"):
+        arrays[k] = torch.empty(n_att, dtype=tdt[spec[k]], device=device)
+    for k in ("a_rowdiff", "a_secleg", "a_padres", "a_timeres"):
+        arrays[k] = torch.empty(n_att - n_trk, dtype=tdt[spec[k]], device=device)
+    ctx = T.tmd_create(geo, BZ)
+    ws = torch.empty(T.tmd_workspace_bytes(ctx, n_trk, n_att, 0), dtype=torch.uint8, device=device)
+    T.tmd_encode_attached(ctx, truth.trk_ncl, truth.trk_qptf, truth.att, truth.leg, arrays, ws,
+                          torch.cuda.current_stream().cuda_stream)
+    T.tmd_destroy(ctx)
+    del truth, ws
+    arrays.update(tf.generate_unattached(geo, n_un, cfg.seed, device, "inv_x", single))
+    torch.cuda.empty_cache()
+    return geo, arrays
+
+
+def sub_frame(arrays: dict, n_bins: int, n_trk_s: int, frac_un: float):
+    """A bounded sample of the workload as host numpy arrays: the first n_trk_s tracks with all their clusters and the
+    first floor(frac_un * count) unattached clusters of every bin (index selection only)."""
+    import torch
+    from tmd_inputs.layout import COMPRESSED_FIELDS, Compressed
+    ncl = (arrays["trk_ncl"][:n_trk_s].to(torch.int64)) & 0xFFFF
+    n_att_s = int(ncl.sum())
+    cnt = arrays["u_bin_count"].to(torch.int64)
+    cnt_s = torch.floor(cnt.to(torch.float64) * frac_un).to(torch.int64)
+    start = torch.cumsum(cnt, 0) - cnt
+    start_s = torch.cumsum(cnt_s, 0) - cnt_s
+    n_un_s = int(cnt_s.sum())
+    bins = torch.repeat_interleave(torch.arange(n_bins, device=cnt.device), cnt_s)
+    idx = start[bins] + (torch.arange(n_un_s, device=cnt.device) - start_s[bins])
+    c = Compressed.empty(n_trk_s, n_att_s, n_un_s, n_bins)
+    for k, (dt, which) in COMPRESSED_FIELDS.items():
+        a = arrays[k]
+        if which == "n_tracks":
+            a = a[:n_trk_s]
+        elif which == "n_attached":
+            a = a[:n_att_s]
+        elif which == "n_residuals":
+            a = a[: n_att_s - n_trk_s]
+        elif which == "n_unattached":
+            a = a[idx]
+        else:
+            a = cnt_s.to(torch.int32)
+        getattr(c, k)[:] = a.cpu().numpy().view(np.dtype(dt))
+    return c
+
+
+def time_oracle(geo, comp) -> float:
+    from oracle import tmd_oracle as O
+    t0 = time.perf_counter()
+    O.decode(geo, BZ, comp)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(geo, arrays, n_trk: int, target_s: float = 12.0) -> dict:
+    """The oracle as it stands (single thread) on a bounded sample: calibrate on a small sample, then ~target_s of work."""
+    probe_trk = max(1, min(n_trk, 2000))
+    c = sub_frame(arrays, geo.n_bins, probe_trk, probe_trk / n_trk)
+    dt = max(time_oracle(geo, c), 1e-4)
+    rate = (c.n_attached + c.n_unattached) / dt
+    frac = min(1.0, target_s * rate / (int(arrays["a_qtot"].shape[0]) + int(arrays["u_qtot"].shape[0])))
+    n_s = max(probe_trk, int(n_trk * frac))
+    c = sub_frame(arrays, geo.n_bins, n_s, n_s / n_trk)
+    dt = time_oracle(geo, c)
+    n_cl = c.n_attached + c.n_unattached
+    return {"value": n_cl / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"first {n_s} of {n_trk} tracks ({c.n_attached} attached) + the same fraction of every bin's unattached "
+                      f"clusters ({c.n_unattached}); oracle/tmd_oracle.c orc_decode, single thread, {dt:.2f} s"}
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = "index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
+        "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        self.p.wait()
+        self.f.seek(0)
+        sm, smax, reasons, power = [], [], set(), []
+        for line in self.f.read().splitlines():
+            v = [x.strip() for x in line.split(",")]
+            if len(v) < 9:
+                continue
+            try:
+                sm.append(float(v[1])); smax.append(float(v[2])); power.append(float(v[3]))
+            except ValueError:
+                continue
+            for name, flag in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), v[5:9]):
+                if flag.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.f.name)
+        # "under load" = samples in the upper half of the power range seen
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": sorted(reasons)}
+        thr = 0.5 * (min(power) + max(power))
+        load = [s for s, p in zip(sm, power) if p >= thr] or sm
+        return {"sm_mhz": float(np.median(load)), "sm_max_mhz": max(smax), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------ arms
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+    from paper_2411_02206_b200 import tmd as T
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+
+    geo, arrays = build_workload(args.workload, device, seed_offset=rank)
+    n_trk, n_att, n_un = (int(arrays[k].shape[0]) for k in ("trk_ncl", "a_qtot", "u_qtot"))
+    n_cl = n_att + n_un
+    ctx = T.tmd_create(geo, BZ)
+    clusters = torch.empty(n_cl * 16, dtype=torch.uint8, device=device)
+    bin_offset = torch.empty(geo.n_bins + 1, dtype=torch.int32, device=device)
+    ws = torch.empty(T.tmd_workspace_bytes(ctx, n_trk, n_att, n_un), dtype=torch.uint8, device=device)
+    comp = T.make_compressed(arrays)
+    out = T.make_output(clusters, bin_offset, ws)
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        T.tmd_decode(ctx, comp, out, 0, stream)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ktimes: dict[str, float] = {}
+    launches = 0
+    for s0, s1 in ev:
+        s0.record()
+        T.tmd_decode(ctx, comp, out, T.TMD_TIMING, stream)
+        s1.record()
+        launches += T.tmd_last_launch_count(ctx)
+        for name, ms in T.tmd_kernel_times(ctx):          # waits for this step's last kernel
+            ktimes[name] = ktimes.get(name, 0.0) + ms
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([total_ms, float(n_cl)], dtype=torch.float64, device=device)
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        total_ms, n_cl_all = float(tmax[0]), float(tsum[1])
+    else:
+        n_cl_all = float(n_cl)
+    ms_per_step = total_ms / args.steps
+    value = n_cl_all / (ms_per_step * 1e-3)
+
+    # ---- end to end: pinned host buffers in, pinned host buffers out, copies inside the timed region
+    h_in = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in arrays.items()}
+    h_clusters = torch.empty(n_cl * 16, dtype=torch.uint8, pin_memory=True)
+    h_binoff = torch.empty(geo.n_bins + 1, dtype=torch.int32, pin_memory=True)
+    h2d = sum(v.numel() * v.element_size() for v in h_in.values())
+    d2h = h_clusters.numel() + h_binoff.numel() * 4
+    del clusters, ws
+    torch.cuda.empty_cache()
+    hcomp = T.make_compressed(h_in)
+    hout = T.make_output(h_clusters, h_binoff)
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    T.tmd_decode_host(ctx, hcomp, hout, 0, stream)            # warm-up (allocates the context's device arena)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        T.tmd_decode_host(ctx, hcomp, hout, 0, stream)        # returns after the stream is synchronised
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = n_cl_all * e2e_steps / float(te[0])
+
+    if rank == 0:
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            pass
+        peak, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
+        kavg = {k: v / args.steps for k, v in ktimes.items()}
+        dom = max(kavg, key=kavg.get)
+        alg = {"decode_attached": algorithmic_bytes_attached(n_trk, n_att),
+               "unattached": algorithmic_bytes_unattached(n_un, geo.n_bins)}.get(dom)
+        achieved = alg / (kavg[dom] * 1e-3) / 1e9 if alg else None
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                    "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(dom, args.workload),
+                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kavg[dom]}
+        total_alg = algorithmic_bytes_attached(n_trk, n_att) + algorithmic_bytes_unattached(n_un, geo.n_bins)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": args.workload, "n_tracks": n_trk, "n_attached": n_att, "n_unattached": n_un,
+                       "sectors_x_rows": "36x152", "bz_tesla": BZ, "l2": "inputs larger than L2, no flush"
+                       if total_alg > 400e6 else "L2-resident workload (flag)", "parallelism": f"replicas x{world}"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "roofline": roofline,
+            "path_gbs": total_alg / (ms_per_step * 1e-3) / 1e9, "path_frac_of_hbm_peak": total_alg / (ms_per_step * 1e-3) / 1e9 / peak,
+            "kernel_ms": kavg,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(geo, arrays, n_trk)
+        print(json.dumps(line), flush=True)
+    T.tmd_destroy(ctx)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """dram bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.txt), else None."""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
+            v = line.split()
+            if len(v) >= 3 and v[0] == workload and v[1] == kernel:
+                return float(v[2])
+    except OSError:
+        pass
+    return None
+
+
+def run_reference(args) -> None:
+    """The CPU oracle, as it stands, on bounded samples of the same workload (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import torch
+    from tmd_inputs import build_geometry, physical as ph, timeframe as tf
+    from oracle import tmd_oracle as O
+
+    geo = build_geometry(36)
+    mk, n_un, single = tf.WORKLOADS[args.workload]
+    cfg = mk()
+    n_s = min(cfg.n_tracks, args.ref_tracks)                          # bounded sample: same mix, fewer tracks
+    frac = n_s / cfg.n_tracks
+    cfg.n_tracks = n_s
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    tr = tf.generate_truth(cfg, geo, dev, batch=200_000)
+    ev_att = tr.att.cpu().numpy().view(ph.CLUSTER_DTYPE).reshape(-1)
+    comp = O.encode(geo, BZ, tr.trk_ncl.cpu().numpy().view(np.uint16), tr.trk_qptf.cpu().numpy(), ev_att, tr.leg.cpu().numpy(),
+                    np.zeros(0, ph.CLUSTER_DTYPE))
+    u = tf.generate_unattached(geo, int(n_un * frac), cfg.seed, dev, "inv_x", single)
+    from tmd_inputs.layout import COMPRESSED_FIELDS, Compressed
+    full = Compressed.empty(comp.n_tracks, comp.n_attached, int(u["u_qtot"].shape[0]), geo.n_bins)
+    for k, (dt, _) in COMPRESSED_FIELDS.items():
+        src = u[k].cpu().numpy().view(np.dtype(dt)) if k in u else getattr(comp, k)
+        getattr(full, k)[:] = src
+    n_cl = full.n_attached + full.n_unattached
+    for _ in range(args.warmup):
+        time_oracle(geo, full)
+    dts = [time_oracle(geo, full) for _ in range(args.steps)]
+    value = n_cl * len(dts) / sum(dts)
+    sample = (f"{n_s} tracks of the {args.workload} mix ({full.n_attached} attached, {full.n_unattached} unattached) per step; "
+              f"oracle/tmd_oracle.c orc_decode, single thread")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(dts) / len(dts), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "sectors_x_rows": "36x152", "bz_tesla": BZ},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }), flush=True)
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4"],
+                    help="c3 = full Pb-Pb-scale time frame, the configuration the metric is quoted on")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-tracks", type=int, default=25_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

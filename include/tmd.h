@@ -135,6 +135,9 @@ typedef struct tmd_ctx tmd_ctx;
                            Without it such inputs are undefined except that nothing is written out of bounds
                            of `clusters` for a decoded sector >= n_sectors_out (the cluster is dropped). */
 
+#define TMD_TIMING 2u   /* record a CUDA event on the stream around every kernel (read back with tmd_kernel_times)   */
+#define TMD_MAX_KERNELS 16
+
 /* Uploads the geometry tables to the current CUDA device.  *out_ctx is set only on success. */
 int tmd_create(const tmd_geometry* geometry, const tmd_field* field, tmd_ctx** out_ctx);
 
@@ -162,6 +165,34 @@ const char* tmd_status_string(int status);
 
 /* Number of kernel launches the last tmd_decode on this context enqueued (for bench.py's gpu_launches). */
 int tmd_last_launch_count(const tmd_ctx* ctx);
+
+/*
+ * Per-kernel device times of the last tmd_decode that ran with TMD_TIMING: waits for that call's last event, then
+ * fills names[i] (static strings) and ms[i] for its kernels in launch order.  Returns the number filled (0 if the last
+ * call did not use TMD_TIMING) or a negative tmd_status.
+ */
+int tmd_kernel_times(tmd_ctx* ctx, int max_kernels, const char** names, float* ms);
+
+/*
+ * Track-model ENCODING of the attached clusters (the synchronous-side step of PAPER.md L68: each coordinate is stored
+ * "as the residual to the correspondent track"; model and formats as above).  DEVICE pointers.
+ * `att` holds the attached clusters in g order (track after track); `leg` the leg index of each inside its track;
+ * trk_qptf the signed curvature / KB in c/GeV.  Writes the trk_* (except trk_ncl) and a_* arrays `out` points to
+ * (as writable device memory; the u_* members are ignored).  `workspace` as for tmd_decode with n_unattached = 0.
+ * Synchronises the stream; TMD_ERR_CORRUPT if sum(trk_ncl) != n_attached, a row/sector is out of range or a track
+ * changes side.
+ */
+typedef struct {
+  uint32_t n_tracks;
+  uint64_t n_attached;
+  const uint16_t* trk_ncl;   /* [n_tracks]   */
+  const float* trk_qptf;     /* [n_tracks]   */
+  const tmd_cluster* att;    /* [n_attached] */
+  const uint8_t* leg;        /* [n_attached] */
+} tmd_attached_truth;
+
+int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compressed* out, void* workspace, size_t workspace_bytes,
+                        void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -6,6 +6,7 @@
 
 #include "tmd_common.cuh"
 #include "tmd_decode.cuh"
+#include "tmd_encode.cuh"
 #include "tmd_rank.cuh"
 #include "tmd_scan.cuh"
 #include "tmd_unattached.cuh"
@@ -17,6 +18,10 @@ struct tmd_ctx {
   RowGeo* d_rows;
   int device;
   int launches;
+  // TMD_TIMING: events[0] before the first kernel, events[i+1] after kernel i of the last tmd_decode
+  cudaEvent_t events[TMD_MAX_KERNELS + 1];
+  const char* kernel_names[TMD_MAX_KERNELS];
+  bool events_created, timing_valid;
   // arena of tmd_decode_host (grown on demand)
   void* arena;
   size_t arena_bytes;
@@ -102,10 +107,14 @@ int check_args(const tmd_ctx* ctx, const tmd_compressed* in, const tmd_output* o
   return TMD_OK;
 }
 
-#define TMD_LAUNCH_CHECK()                           \
-  do {                                               \
-    ctx->launches++;                                 \
-    if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA; \
+#define TMD_LAUNCH_CHECK(name)                                                                  \
+  do {                                                                                          \
+    if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA;                                 \
+    if (timing && ctx->launches < TMD_MAX_KERNELS) {                                            \
+      ctx->kernel_names[ctx->launches] = name;                                                  \
+      if (cudaEventRecord(ctx->events[ctx->launches + 1], st) != cudaSuccess) return TMD_ERR_CUDA; \
+    }                                                                                           \
+    ctx->launches++;                                                                            \
   } while (0)
 
 }  // namespace
@@ -183,21 +192,30 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   uint16_t* d_hist = (uint16_t*)(ws + W.o_hist);
   uint32_t* d_rel = (uint32_t*)(ws + W.o_rel);
   uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
-  const bool validate = (flags & TMD_VALIDATE) != 0;
+  const bool validate = (flags & TMD_VALIDATE) != 0, timing = (flags & TMD_TIMING) != 0;
   ctx->launches = 0;
+  ctx->timing_valid = false;
+  if (timing) {
+    if (!ctx->events_created) {
+      for (int i = 0; i <= TMD_MAX_KERNELS; ++i)
+        if (cudaEventCreate(&ctx->events[i]) != cudaSuccess) return TMD_ERR_CUDA;
+      ctx->events_created = true;
+    }
+    if (cudaEventRecord(ctx->events[0], st) != cudaSuccess) return TMD_ERR_CUDA;
+  }
   if (cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
 
   if (n_trk > 0) {  // A1: track offsets + chunk table
     k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("track_tile_sums");
     k_scan_tile_sums<<<1, 1024, 0, st>>>(d_tile, W.n_tiles);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("scan_tile_sums");
     k_track_offsets<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile, W.n_tiles, d_off);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("track_offsets");
   }
   if (validate) {
     k_validate<<<148, 256, 0, st>>>(G, *in, d_off, d_err);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("validate");
     uint32_t h_err[ERR_WORDS];
     if (cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
@@ -205,7 +223,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   }
   if (n_trk > 0) {
     k_chunk_table<<<(n_trk + 1 + 255) / 256, 256, 0, st>>>(d_off, n_trk, d_cfirst, W.n_chunks);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("chunk_table");
     // A3: walk + per-chunk histogram + ranks
     RankArgs R;
     R.off = d_off; R.chunk_first = d_cfirst; R.trk_row0 = in->trk_row0; R.trk_sec0 = in->trk_sec0;
@@ -213,43 +231,99 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     R.n_chunks = W.n_chunks; R.n_tracks = n_trk; R.n_attached = n_att;
     const size_t rank_smem = CHUNK_WINDOW * 4 + (size_t)n_bins * 8;
     k_rank<<<W.n_chunks, RANK_THREADS, rank_smem, st>>>(G, R);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("rank");
     // A4: column scan over chunks
     dim3 cg((n_bins + 255) / 256, W.n_groups);
     k_col_group_sums<<<cg, 256, 0, st>>>(d_hist, W.n_chunks, n_bins, d_gsum);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("col_group_sums");
     k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, st>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("col_group_scan");
   } else {
     if (cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
   }
   k_bin_offsets<<<1, 1024, 0, st>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
-  TMD_LAUNCH_CHECK();
+  TMD_LAUNCH_CHECK("bin_offsets");
   if (n_trk > 0) {
     dim3 cg((n_bins + 255) / 256, W.n_groups);
     k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("col_apply");
     // A5 + A6
     DecodeArgs D;
     D.off = d_off; D.rel = d_rel; D.rank16 = d_rank; D.in = *in; D.clusters = (uint4*)out->clusters;
     D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
     D.n_clusters_total = n_att + n_un;
     k_decode_attached<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, sizeof(RowGeo) * G.n_rows, st>>>(G, D);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("decode_attached");
   }
   if (n_un > 0) {  // A7
     UnattachedArgs U;
     U.in = *in; U.u_start = d_ustart; U.bin_offset = out->bin_offset; U.att_cnt = d_attcnt;
     U.clusters = (uint4*)out->clusters; U.n_clusters_total = n_att + n_un;
     k_unattached<<<n_bins, UNATT_THREADS, 0, st>>>(G, U);
-    TMD_LAUNCH_CHECK();
+    TMD_LAUNCH_CHECK("unattached");
   }
+  ctx->timing_valid = timing;
   if (validate) {
     uint32_t h_err[ERR_WORDS];
     if (cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
     if (h_err[ERR_TRACK_FIELD] || h_err[ERR_SECTOR_OUT]) return TMD_ERR_CORRUPT;
   }
+  return TMD_OK;
+}
+
+int tmd_kernel_times(tmd_ctx* ctx, int max_kernels, const char** names, float* ms) {
+  if (!ctx || !names || !ms || max_kernels < 0) return TMD_ERR_ARG;
+  if (!ctx->timing_valid) return 0;
+  const int n = ctx->launches < TMD_MAX_KERNELS ? ctx->launches : TMD_MAX_KERNELS;
+  if (n > 0 && cudaEventSynchronize(ctx->events[n]) != cudaSuccess) return TMD_ERR_CUDA;
+  int k = 0;
+  for (; k < n && k < max_kernels; ++k) {
+    names[k] = ctx->kernel_names[k];
+    if (cudaEventElapsedTime(&ms[k], ctx->events[k], ctx->events[k + 1]) != cudaSuccess) return TMD_ERR_CUDA;
+  }
+  return k;
+}
+
+int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compressed* out, void* workspace, size_t workspace_bytes,
+                        void* cuda_stream) {
+  if (!ctx || !in || !out) return TMD_ERR_ARG;
+  if (in->n_attached >= (1ull << 32) || in->n_attached < in->n_tracks) return TMD_ERR_ARG;
+  if (in->n_tracks == 0) return in->n_attached == 0 ? TMD_OK : TMD_ERR_ARG;
+  if (!in->trk_ncl || !in->trk_qptf || !in->att || !in->leg) return TMD_ERR_ARG;
+  void* outs[] = {(void*)out->trk_qpt, (void*)out->trk_row0, (void*)out->trk_sec0, (void*)out->trk_pad0, (void*)out->trk_time0,
+                  (void*)out->a_qtot, (void*)out->a_qmax, (void*)out->a_flags, (void*)out->a_sigpad, (void*)out->a_sigtime};
+  for (void* p : outs) if (!p) return TMD_ERR_ARG;
+  if (in->n_attached > in->n_tracks && (!out->a_rowdiff || !out->a_secleg || !out->a_padres || !out->a_timeres)) return TMD_ERR_ARG;
+  if (misaligned(in->trk_ncl, 16) || misaligned(in->att, 16)) return TMD_ERR_ALIGN;
+  const Workspace W = layout(ctx->geo.n_bins, in->n_tracks, in->n_attached);
+  if (!workspace || workspace_bytes < W.total) return TMD_ERR_WORKSPACE;
+  if (misaligned(workspace, ALIGN)) return TMD_ERR_ALIGN;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)workspace;
+  uint32_t* d_err = (uint32_t*)(ws + W.o_err);
+  uint32_t* d_tile = (uint32_t*)(ws + W.o_tile_sum);
+  uint32_t* d_off = (uint32_t*)(ws + W.o_off);
+  if (cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+  k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, in->n_tracks, d_tile);
+  k_scan_tile_sums<<<1, 1024, 0, st>>>(d_tile, W.n_tiles);
+  k_track_offsets<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, in->n_tracks, d_tile, W.n_tiles, d_off);
+  EncodeArgs E;
+  E.n_tracks = in->n_tracks; E.off = d_off; E.trk_qptf = in->trk_qptf; E.att = (const uint4*)in->att; E.leg = in->leg;
+  E.trk_qpt = (int8_t*)out->trk_qpt; E.trk_row0 = (uint8_t*)out->trk_row0; E.trk_sec0 = (uint8_t*)out->trk_sec0;
+  E.trk_pad0 = (uint16_t*)out->trk_pad0; E.trk_time0 = (uint32_t*)out->trk_time0;
+  E.a_qtot = (uint16_t*)out->a_qtot; E.a_qmax = (uint16_t*)out->a_qmax; E.a_flags = (uint8_t*)out->a_flags;
+  E.a_sigpad = (uint8_t*)out->a_sigpad; E.a_sigtime = (uint8_t*)out->a_sigtime;
+  E.a_rowdiff = (uint8_t*)out->a_rowdiff; E.a_secleg = (uint8_t*)out->a_secleg;
+  E.a_padres = (uint16_t*)out->a_padres; E.a_timeres = (uint32_t*)out->a_timeres;
+  E.err = d_err;
+  k_encode_attached<<<(in->n_tracks + 127) / 128, 128, sizeof(RowGeo) * ctx->geo.n_rows, st>>>(ctx->geo, E);
+  if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA;
+  uint32_t h_err[ERR_WORDS + 1];
+  if (cudaMemcpyAsync(h_err, d_err, ERR_WORDS * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
+  if (cudaMemcpyAsync(&h_err[ERR_WORDS], d_off + in->n_tracks, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+  if (h_err[ERR_TRACK_FIELD] || h_err[ERR_WORDS] != (uint32_t)in->n_attached) return TMD_ERR_CORRUPT;
   return TMD_OK;
 }
 
@@ -317,6 +391,8 @@ int tmd_destroy(tmd_ctx* ctx) {
   if (!ctx) return TMD_OK;
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->d_rows) cudaFree(ctx->d_rows);
+  if (ctx->events_created)
+    for (int i = 0; i <= TMD_MAX_KERNELS; ++i) cudaEventDestroy(ctx->events[i]);
   delete ctx;
   return TMD_OK;
 }

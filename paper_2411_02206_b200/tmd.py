@@ -17,6 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 
 TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT = 0, -1, -2, -3, -4, -5
 TMD_VALIDATE = 1
+TMD_TIMING = 2
+TMD_MAX_KERNELS = 16
 PROBE_FINAL = 0xFFFFFFFF
 
 # (field name, numpy dtype) in the order of struct tmd_compressed
@@ -49,6 +51,11 @@ class tmd_output(C.Structure):
                 ("probe_step", C.c_uint32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
+class tmd_attached_truth(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint32), ("n_attached", C.c_uint64), ("trk_ncl", C.c_void_p), ("trk_qptf", C.c_void_p),
+                ("att", C.c_void_p), ("leg", C.c_void_p)]
+
+
 _lib = None
 
 
@@ -66,6 +73,11 @@ def lib() -> C.CDLL:
         L.tmd_status_string.argtypes = [C.c_int]
         L.tmd_status_string.restype = C.c_char_p
         L.tmd_last_launch_count.argtypes = [C.c_void_p]
+        L.tmd_kernel_times.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+        L.tmd_encode_attached.argtypes = [C.c_void_p, C.POINTER(tmd_attached_truth), C.POINTER(tmd_compressed), C.c_void_p,
+                                          C.c_size_t, C.c_void_p]
+        L.tmd_kernel_times.restype = C.c_int
+        L.tmd_encode_attached.restype = C.c_int
         for f in (L.tmd_create, L.tmd_workspace_bytes, L.tmd_decode, L.tmd_decode_host, L.tmd_destroy, L.tmd_last_launch_count):
             f.restype = C.c_int
         _lib = L
@@ -148,3 +160,24 @@ def tmd_decode(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, 
 def tmd_decode_host(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, stream: int = 0) -> None:
     """End-to-end decode with HOST pointers (copies in, decodes, copies out, synchronises)."""
     _check(lib().tmd_decode_host(ctx, C.byref(comp), C.byref(out), flags, stream))
+
+
+def tmd_kernel_times(ctx: int) -> list[tuple[str, float]]:
+    """(kernel name, milliseconds) of the last tmd_decode that ran with TMD_TIMING, in launch order."""
+    names = (C.c_char_p * TMD_MAX_KERNELS)()
+    ms = (C.c_float * TMD_MAX_KERNELS)()
+    n = lib().tmd_kernel_times(ctx, TMD_MAX_KERNELS, names, ms)
+    if n < 0:
+        raise TmdError(n)
+    return [(names[i].decode(), float(ms[i])) for i in range(n)]
+
+
+def tmd_encode_attached(ctx: int, trk_ncl, trk_qptf, att, leg, out_arrays: dict, workspace, stream: int = 0) -> None:
+    """Encode g-ordered attached clusters (DEVICE tensors) into the trk_* / a_* arrays of `out_arrays` (DEVICE, writable)."""
+    truth = tmd_attached_truth(int(trk_ncl.shape[0]), int(leg.shape[0]), _ptr(trk_ncl), _ptr(trk_qptf), _ptr(att), _ptr(leg))
+    c = tmd_compressed(truth.n_tracks, truth.n_attached, 0)
+    for k, _ in COMPRESSED_ARRAYS:
+        if k in out_arrays:
+            setattr(c, k, _ptr(out_arrays[k]))
+    ws_bytes = int(workspace.numel() * workspace.element_size())
+    _check(lib().tmd_encode_attached(ctx, C.byref(truth), C.byref(c), _ptr(workspace), ws_bytes, stream))

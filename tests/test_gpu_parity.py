@@ -154,3 +154,43 @@ def test_validate_flag_reports_corrupt_counts():
     with pytest.raises(T.TmdError) as e:
         gpu_decode(geo2, BZ, c2, flags=T.TMD_VALIDATE)
     assert e.value.status == T.TMD_ERR_CORRUPT
+
+
+def test_gpu_encoder_matches_oracle_encoder(phys_case):
+    # tmd_encode_attached (the synchronous-side step) produces the oracle encoder's bytes
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    from gpu_util import _as_torch
+    name, geo, ev, comp = phys_case
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        dev = lambda a: _as_torch(np.ascontiguousarray(a)).cuda()
+        att = torch.from_numpy(np.ascontiguousarray(ev.att).view(np.int32).reshape(-1, 4)).cuda()
+        out = {}
+        for k in ("trk_qpt", "trk_row0", "trk_sec0", "trk_pad0", "trk_time0", "a_qtot", "a_qmax", "a_flags", "a_sigpad", "a_sigtime",
+                  "a_rowdiff", "a_secleg", "a_padres", "a_timeres"):
+            out[k] = torch.zeros_like(dev(getattr(comp, k)))
+        ws = torch.empty(T.tmd_workspace_bytes(ctx, comp.n_tracks, comp.n_attached, 0), dtype=torch.uint8, device="cuda")
+        T.tmd_encode_attached(ctx, dev(ev.trk_ncl), dev(ev.trk_qptf), att, dev(ev.leg), out, ws, torch.cuda.current_stream().cuda_stream)
+        for k, v in out.items():
+            want = getattr(comp, k)
+            got = v.cpu().numpy().view(want.dtype)
+            assert np.array_equal(got, want), f"{k}: " + first_mismatch(got, want)
+    finally:
+        T.tmd_destroy(ctx)
+
+
+def test_bench_workload_builder_matches_oracle():
+    # the path bench.py times: torch helix truth -> GPU encoder -> GPU decoder, against the oracle on the same arrays
+    import torch
+    import bench
+    from tmd_inputs import timeframe as tf
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    saved = tf.WORKLOADS["c1"]
+    geo, arrays = bench.build_workload("c1", torch.device("cuda", 0))
+    comp = Compressed.empty(int(arrays["trk_ncl"].shape[0]), int(arrays["a_qtot"].shape[0]), int(arrays["u_qtot"].shape[0]), geo.n_bins)
+    for k, (dt, _) in COMPRESSED_FIELDS.items():
+        getattr(comp, k)[:] = arrays[k].cpu().numpy().view(np.dtype(dt))
+    assert comp.n_tracks == 10_000 and 1.1e6 < comp.n_attached < 1.4e6
+    assert_same(gpu_decode(geo, BZ, comp, probe_step=0xFFFFFFFF), O.decode(geo, BZ, comp, probe_step=0xFFFFFFFF))
+    assert tf.WORKLOADS["c1"] is saved
