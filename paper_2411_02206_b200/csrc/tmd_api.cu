@@ -9,6 +9,8 @@
 #include "tmd_encode.cuh"
 #include "tmd_rank.cuh"
 #include "tmd_scan.cuh"
+#include "tmd_scatter.cuh"
+#include "tmd_sort.cuh"
 #include "tmd_unattached.cuh"
 
 using namespace tmd;
@@ -25,6 +27,7 @@ struct tmd_ctx {
   // arena of tmd_decode_host (grown on demand)
   void* arena;
   size_t arena_bytes;
+  size_t decode_smem;
 };
 
 namespace {
@@ -34,7 +37,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
 struct Workspace {
   uint32_t n_tiles, n_chunks, n_groups;
-  size_t o_err, o_tile_sum, o_off, o_chunk_first, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, total;
+  size_t o_err, o_tile_sum, o_off, o_len, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
 };
 
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
@@ -47,13 +50,15 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   w.o_err = take(ERR_WORDS * 4);
   w.o_tile_sum = take(((size_t)w.n_tiles + 1) * 4);
   w.o_off = take(((size_t)n_tracks + 1) * 4);
-  w.o_chunk_first = take(((size_t)w.n_chunks + 1) * 4);
+  w.o_len = take((size_t)LEN_BINS * 4 * 3);             // len_hist, len_base, len_cursor
+  w.o_perm = take((size_t)n_tracks * 4);
   w.o_att_cnt = take((size_t)n_bins * 4);
   w.o_u_start = take(((size_t)n_bins + 1) * 4);
   w.o_gsum = take((size_t)w.n_groups * n_bins * 4);
   w.o_hist = take((size_t)w.n_chunks * n_bins * 2);
   w.o_rel = take((size_t)w.n_chunks * n_bins * 4);
   w.o_rank16 = take((size_t)n_att * 2);
+  w.o_inter = take((size_t)n_att * 8);
   w.total = o;
   return w;
 }
@@ -145,6 +150,9 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(CHUNK_WINDOW * 4 + (size_t)g->n_sectors_out * g->n_rows * 8));
+  ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_track_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
   if (e != cudaSuccess) {
     cudaGetLastError();
     if (ctx->d_rows) cudaFree(ctx->d_rows);
@@ -185,13 +193,15 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   uint32_t* d_err = (uint32_t*)(ws + W.o_err);
   uint32_t* d_tile = (uint32_t*)(ws + W.o_tile_sum);
   uint32_t* d_off = (uint32_t*)(ws + W.o_off);
-  uint32_t* d_cfirst = (uint32_t*)(ws + W.o_chunk_first);
+  uint32_t* d_len = (uint32_t*)(ws + W.o_len);
+  uint32_t* d_perm = (uint32_t*)(ws + W.o_perm);
   uint32_t* d_attcnt = (uint32_t*)(ws + W.o_att_cnt);
   uint32_t* d_ustart = (uint32_t*)(ws + W.o_u_start);
   uint32_t* d_gsum = (uint32_t*)(ws + W.o_gsum);
   uint16_t* d_hist = (uint16_t*)(ws + W.o_hist);
   uint32_t* d_rel = (uint32_t*)(ws + W.o_rel);
   uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
+  uint2* d_inter = (uint2*)(ws + W.o_inter);
   const bool validate = (flags & TMD_VALIDATE) != 0, timing = (flags & TMD_TIMING) != 0;
   ctx->launches = 0;
   ctx->timing_valid = false;
@@ -222,13 +232,24 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;
   }
   if (n_trk > 0) {
-    k_chunk_table<<<(n_trk + 1 + 255) / 256, 256, 0, st>>>(d_off, n_trk, d_cfirst, W.n_chunks);
-    TMD_LAUNCH_CHECK("chunk_table");
-    // A3: walk + per-chunk histogram + ranks
+    // A2: load-balance order (counting sort by cluster count, longest first)
+    if (cudaMemsetAsync(d_len, 0, LEN_BINS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+    const uint32_t sort_blocks = (n_trk + SORT_TILE - 1) / SORT_TILE;
+    k_len_hist<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len);
+    TMD_LAUNCH_CHECK("len_hist");
+    k_len_scan<<<1, 1024, 0, st>>>(d_len, d_len + LEN_BINS, d_len + 2 * LEN_BINS);
+    TMD_LAUNCH_CHECK("len_scan");
+    k_len_perm<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len + LEN_BINS, d_len + 2 * LEN_BINS, d_perm);
+    TMD_LAUNCH_CHECK("len_perm");
+    // A3 (walk) + A5: track-model decode -> intermediate records in g order
+    DecodeArgs D;
+    D.off = d_off; D.perm = d_perm; D.in = *in; D.inter = d_inter;
+    D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
+    k_track_decode<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
+    TMD_LAUNCH_CHECK("track_decode");
+    // A3 (count): per-chunk histogram + ranks
     RankArgs R;
-    R.off = d_off; R.chunk_first = d_cfirst; R.trk_row0 = in->trk_row0; R.trk_sec0 = in->trk_sec0;
-    R.a_rowdiff = in->a_rowdiff; R.a_secleg = in->a_secleg; R.hist = d_hist; R.rank16 = d_rank;
-    R.n_chunks = W.n_chunks; R.n_tracks = n_trk; R.n_attached = n_att;
+    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att;
     const size_t rank_smem = CHUNK_WINDOW * 4 + (size_t)n_bins * 8;
     k_rank<<<W.n_chunks, RANK_THREADS, rank_smem, st>>>(G, R);
     TMD_LAUNCH_CHECK("rank");
@@ -247,13 +268,13 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     dim3 cg((n_bins + 255) / 256, W.n_groups);
     k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
     TMD_LAUNCH_CHECK("col_apply");
-    // A5 + A6
-    DecodeArgs D;
-    D.off = d_off; D.rel = d_rel; D.rank16 = d_rank; D.in = *in; D.clusters = (uint4*)out->clusters;
-    D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
-    D.n_clusters_total = n_att + n_un;
-    k_decode_attached<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, sizeof(RowGeo) * G.n_rows, st>>>(G, D);
-    TMD_LAUNCH_CHECK("decode_attached");
+    // A6: copy-through + scatter
+    ScatterArgs S;
+    S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
+    S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
+    S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un;
+    k_scatter<<<(n_att + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, 0, st>>>(G, S);
+    TMD_LAUNCH_CHECK("scatter");
   }
   if (n_un > 0) {  // A7
     UnattachedArgs U;

@@ -1,6 +1,6 @@
-// tmd_rank.cuh -- A3: geometry walk of the attached clusters, per-chunk histogram over bins and the rank of every
-// attached cluster among the clusters of its chunk that fall in the same bin (ascending global attached index g).
-// Integer only: the (sector,row) sequence of a track depends on the a_rowdiff / a_secleg streams alone.
+// tmd_rank.cuh -- A3 (count part): per-chunk histogram over bins and the rank of every attached cluster among the
+// clusters of its chunk that fall in the same bin (ascending global attached index g).  Integer only.  The bins come
+// from the geometry walk of the track-decode kernel (tmd_decode.cuh), which leaves bin(g) in its intermediate records.
 //
 // Together with the column scan (tmd_scan.cuh) this yields the canonical position of every attached cluster
 // (DESIGN.md §3 reading 11):   position(g) = rel[chunk][bin] + rank16[g].
@@ -12,21 +12,15 @@
 namespace tmd {
 
 struct RankArgs {
-  const uint32_t* off;          // [n_tracks+1]
-  const uint32_t* chunk_first;  // [n_chunks+1]
-  const uint8_t* trk_row0;
-  const uint8_t* trk_sec0;
-  const uint8_t* a_rowdiff;
-  const uint8_t* a_secleg;
+  const uint2* inter;           // [n_attached] intermediate records of the track-decode kernel; bin = .y >> 16
   uint16_t* hist;               // [n_chunks][n_bins]
   uint16_t* rank16;             // [n_attached]
-  uint32_t n_chunks, n_tracks, n_attached;
+  uint32_t n_attached;
 };
 
 constexpr int RANK_THREADS = 1024;
 
-// One block per chunk c = the attached clusters g in [c << CHUNK_SHIFT, (c+1) << CHUNK_SHIFT).  A track that straddles the
-// window start is walked from its first cluster, but only clusters inside the window are recorded.
+// One block per chunk c = the attached clusters g in [c << CHUNK_SHIFT, (c+1) << CHUNK_SHIFT).
 // Dynamic shared memory: bin_of[CHUNK_WINDOW] u16, list[CHUNK_WINDOW] u16, cnt[n_bins] u32, start[n_bins] u32.
 __global__ void __launch_bounds__(RANK_THREADS, 1) k_rank(DevGeo G, RankArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -40,30 +34,9 @@ __global__ void __launch_bounds__(RANK_THREADS, 1) k_rank(DevGeo G, RankArgs A) 
   const uint32_t w0 = c << CHUNK_SHIFT;
   const uint32_t w1 = min(w0 + CHUNK_WINDOW, A.n_attached);
   const uint32_t n = w1 - w0;
-  uint32_t tA = A.chunk_first[c];
-  const uint32_t tB = A.chunk_first[c + 1];
-  if (tA == A.n_tracks || A.off[tA] != w0) tA -= 1;   // the track that straddles the window start
   for (uint32_t b = tid; b < n_bins; b += nth) cnt[b] = 0;
-
-  // 1. walk: one thread per track, bins in g order into shared memory
-  for (uint32_t t = tA + tid; t < tB; t += nth) {
-    const uint32_t gf = A.off[t], ncl = A.off[t + 1] - gf;
-    WalkState w;
-    const uint32_t sec0 = A.trk_sec0[t];
-    w.row = A.trk_row0[t];
-    w.side = sec0 / G.n_az;
-    w.az = sec0 - w.side * G.n_az;
-    w.dir = +1;
-    if (gf >= w0) bin_of[gf - w0] = sec0 < G.n_sectors_out ? (uint16_t)(sec0 * G.n_rows + w.row) : BIN_INVALID;
-    const uint8_t* rd = A.a_rowdiff + (gf - t);   // residual index of cluster j: off[t] - t + j - 1
-    const uint8_t* sl = A.a_secleg + (gf - t);
-    const uint32_t j_end = min(ncl, w1 - gf);      // clusters at or beyond w1 belong to the next chunk
-    for (uint32_t j = 1; j < j_end; ++j) {
-      walk_step(w, rd[j - 1], sl[j - 1], G.n_rows, G.n_az);
-      const uint32_t sec = w.side * G.n_az + w.az;
-      if (gf + j >= w0) bin_of[gf + j - w0] = sec < G.n_sectors_out ? (uint16_t)(sec * G.n_rows + w.row) : BIN_INVALID;
-    }
-  }
+  // 1. bins of the chunk's clusters in g order (the geometry walk A3 ran inside the track-decode kernel)
+  for (uint32_t i = tid; i < n; i += nth) bin_of[i] = (uint16_t)(A.inter[w0 + i].y >> 16);
   __syncthreads();
   // 2. histogram of the chunk
   for (uint32_t i = tid; i < n; i += nth) {
