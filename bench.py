@@ -42,6 +42,14 @@ def algorithmic_bytes_unattached(n_un: int, n_bins: int) -> int:
     return 13 * n_un + 4 * n_bins + 16 * n_un + 4 * (n_bins + 1)
 
 
+def kernel_algorithmic_bytes(n_trk: int, n_att: int, n_un: int, n_bins: int) -> dict:
+    """The share of the algorithmic bytes each kernel is there to move: the decode kernel consumes the
+    per-track fields and the four residual streams, the scatter kernel the copy-through fields and writes the records,
+    the unattached kernel its 13 B in / 16 B out.  The walk/rank and scan kernels move no algorithmic byte (overhead)."""
+    return {"track_decode": 11 * n_trk + 8 * (n_att - n_trk), "scatter": 7 * n_att + 16 * n_att,
+            "unattached": algorithmic_bytes_unattached(n_un, n_bins)}
+
+
 # ------------------------------------------------------------------------------------------------ workload on the device
 def build_workload(name: str, device, seed_offset: int = 0):
     """Synthetic time frame `name` (tmd_inputs.timeframe.WORKLOADS) as device tensors of the compressed SoA.
@@ -132,42 +140,53 @@ def cpu_baseline(geo, arrays, n_trk: int, target_s: float = 12.0) -> dict:
 
 # ------------------------------------------------------------------------------------------------ clocks
 class ClockSampler:
-    Q = "index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
-        "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    """SM clock, power and throttle reasons sampled through NVML every few milliseconds DURING the timed region."""
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4}
 
-    def __init__(self, gpu_index: int):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    def __init__(self, gpu_index: int, period_s: float = 0.004):
+        import threading
+        self.samples, self.err, self.stop_flag, self.period = [], None, False, period_s
         try:
-            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
-                                       "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
-        except OSError:
-            self.p = None
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[gpu_index]) if vis and vis.split(",")[gpu_index].isdigit() else gpu_index
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # noqa: BLE001 -- no NVML: report it in the JSON line
+            self.err = f"nvml unavailable: {e}"
+            return
+        self.th = threading.Thread(target=self._run, daemon=True)
+        self.th.start()
+
+    def _run(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                self.samples.append((float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)),
+                                     nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0,
+                                     int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))))
+            except Exception as e:  # noqa: BLE001
+                self.err = f"nvml sample failed: {e}"
+                return
+            time.sleep(self.period)
 
     def stop(self) -> dict:
-        if self.p is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.p.terminate()
-        self.p.wait()
-        self.f.seek(0)
-        sm, smax, reasons, power = [], [], set(), []
-        for line in self.f.read().splitlines():
-            v = [x.strip() for x in line.split(",")]
-            if len(v) < 9:
-                continue
-            try:
-                sm.append(float(v[1])); smax.append(float(v[2])); power.append(float(v[3]))
-            except ValueError:
-                continue
-            for name, flag in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), v[5:9]):
-                if flag.lower().startswith("active"):
-                    reasons.add(name)
-        os.unlink(self.f.name)
-        # "under load" = samples in the upper half of the power range seen
-        if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": sorted(reasons)}
-        thr = 0.5 * (min(power) + max(power))
-        load = [s for s, p in zip(sm, power) if p >= thr] or sm
-        return {"sm_mhz": float(np.median(load)), "sm_max_mhz": max(smax), "reasons": sorted(reasons), "samples": len(sm)}
+        if self.err and not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [self.err]}
+        self.stop_flag = True
+        self.th.join()
+        sm = [x[0] for x in self.samples]
+        power = [x[1] for x in self.samples]
+        mask = 0
+        for x in self.samples:
+            mask |= x[2]
+        reasons = sorted(k for k, b in {**self.BAD, **self.NOTE}.items() if mask & b)
+        thr = 0.5 * (min(power) + max(power))          # "under load" = samples in the upper half of the power range seen
+        load = [c for c, p in zip(sm, power) if p >= thr] or sm
+        return {"sm_mhz": float(np.median(load)), "sm_max_mhz": self.sm_max, "reasons": reasons, "samples": len(sm),
+                "power_w_max": max(power)}
 
 
 # ------------------------------------------------------------------------------------------------ arms
@@ -226,6 +245,15 @@ def run_ours(args) -> None:
         n_cl_all = float(n_cl)
     ms_per_step = total_ms / args.steps
     value = n_cl_all / (ms_per_step * 1e-3)
+    # ---- outside the timed region: the same step with every kernel alone on one stream (TMD_SERIAL), for the
+    #      per-kernel times without overlap that the roofline of the dominant kernel is computed from
+    kserial: dict[str, float] = {}
+    n_serial = 3
+    for _ in range(n_serial):
+        T.tmd_decode(ctx, comp, out, T.TMD_TIMING | T.TMD_SERIAL, stream)
+        for name, ms in T.tmd_kernel_times(ctx):
+            kserial[name] = kserial.get(name, 0.0) + ms / n_serial
+    torch.cuda.synchronize()
 
     # ---- end to end: pinned host buffers in, pinned host buffers out, copies inside the timed region
     h_in = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in arrays.items()}
@@ -257,13 +285,16 @@ def run_ours(args) -> None:
             pass
         peak, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
         kavg = {k: v / args.steps for k, v in ktimes.items()}
-        dom = max(kavg, key=kavg.get)
-        alg = {"decode_attached": algorithmic_bytes_attached(n_trk, n_att),
-               "unattached": algorithmic_bytes_unattached(n_un, geo.n_bins)}.get(dom)
-        achieved = alg / (kavg[dom] * 1e-3) / 1e9 if alg else None
+        kalg = kernel_algorithmic_bytes(n_trk, n_att, n_un, geo.n_bins)
+        dom = max(kserial, key=kserial.get)
+        alg = kalg.get(dom)
+        achieved = alg / (kserial[dom] * 1e-3) / 1e9 if alg else None
         roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                     "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(dom, args.workload),
-                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kavg[dom]}
+                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kserial[dom],
+                    "kernel_ms_in_timed_region": kavg.get(dom),
+                    "note": "kernel timed alone on one stream (TMD_SERIAL pass after the timed region); in the timed region "
+                            "it overlaps the integer kernels of the second stream"}
         total_alg = algorithmic_bytes_attached(n_trk, n_att) + algorithmic_bytes_unattached(n_un, geo.n_bins)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -277,7 +308,8 @@ def run_ours(args) -> None:
             "clocks": clocks,
             "roofline": roofline,
             "path_gbs": total_alg / (ms_per_step * 1e-3) / 1e9, "path_frac_of_hbm_peak": total_alg / (ms_per_step * 1e-3) / 1e9 / peak,
-            "kernel_ms": kavg,
+            "kernel_ms": kavg, "kernel_ms_serial": kserial,
+            "kernel_gbs_serial": {k: kalg[k] / (kserial[k] * 1e-3) / 1e9 for k in kalg if k in kserial},
         }
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(geo, arrays, n_trk)

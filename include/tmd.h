@@ -135,8 +135,9 @@ typedef struct tmd_ctx tmd_ctx;
                            Without it such inputs are undefined except that nothing is written out of bounds
                            of `clusters` for a decoded sector >= n_sectors_out (the cluster is dropped). */
 
-#define TMD_TIMING 2u   /* record a CUDA event on the stream around every kernel (read back with tmd_kernel_times)   */
-#define TMD_MAX_KERNELS 16
+#define TMD_TIMING 2u   /* record a CUDA event pair around every kernel, on the stream it runs on (tmd_kernel_times)      */
+#define TMD_SERIAL 4u   /* run every kernel on `cuda_stream` alone (no second stream): per-kernel times without overlap */
+#define TMD_MAX_KERNELS 24
 
 /* Uploads the geometry tables to the current CUDA device.  *out_ctx is set only on success. */
 int tmd_create(const tmd_geometry* geometry, const tmd_field* field, tmd_ctx** out_ctx);
@@ -145,9 +146,12 @@ int tmd_create(const tmd_geometry* geometry, const tmd_field* field, tmd_ctx** o
 int tmd_workspace_bytes(const tmd_ctx* ctx, uint32_t n_tracks, uint64_t n_attached, uint64_t n_unattached, size_t* out_bytes);
 
 /*
- * Decode one time frame (rows A1-A7).  Only enqueues kernels on `cuda_stream` (a cudaStream_t; null = default stream)
- * and returns; no allocation, no host synchronisation and no device-to-host copy unless TMD_VALIDATE is set.
- * Results are valid once the stream has been synchronised.  Concurrent calls need distinct workspaces.
+ * Decode one time frame (rows A1-A7).  Only enqueues work and returns; no allocation, no host synchronisation and no
+ * device-to-host copy unless TMD_VALIDATE is set.  The floating-point track decode (A5) and the scatter (A6) run on
+ * `cuda_stream` (a cudaStream_t; null = default stream); the integer side (A3 walk and ranks, A4, A7) runs on a second
+ * stream owned by the context, forked from and joined back into `cuda_stream` with events, so for the caller the call
+ * behaves like work enqueued on `cuda_stream`: results are valid once that stream has been synchronised.
+ * Concurrent calls need distinct contexts and workspaces.
  */
 int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream);
 

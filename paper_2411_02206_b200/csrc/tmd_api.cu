@@ -20,14 +20,19 @@ struct tmd_ctx {
   RowGeo* d_rows;
   int device;
   int launches;
-  // TMD_TIMING: events[0] before the first kernel, events[i+1] after kernel i of the last tmd_decode
-  cudaEvent_t events[TMD_MAX_KERNELS + 1];
+  // Second stream of tmd_decode: the integer side of the path (walk + ranks, column scan, bin offsets, unattached
+  // clusters) runs there, concurrently with the floating-point track decode on the caller's stream.
+  cudaStream_t side;
+  cudaEvent_t ev_fork, ev_rel, ev_join;
+  // TMD_TIMING: one event pair around every kernel of the last tmd_decode, recorded on the stream it ran on
+  cudaEvent_t ev_t0[TMD_MAX_KERNELS], ev_t1[TMD_MAX_KERNELS];
   const char* kernel_names[TMD_MAX_KERNELS];
   bool events_created, timing_valid;
   // arena of tmd_decode_host (grown on demand)
   void* arena;
   size_t arena_bytes;
-  size_t decode_smem;
+  size_t decode_smem, rank_smem;
+  int n_sm;
 };
 
 namespace {
@@ -36,8 +41,8 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
 struct Workspace {
-  uint32_t n_tiles, n_chunks, n_groups;
-  size_t o_err, o_tile_sum, o_off, o_len, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
+  uint32_t n_tiles, n_chunks, n_groups, n_sub;
+  size_t o_err, o_tile_sum, o_off, o_sub_first, o_len, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
 };
 
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
@@ -45,11 +50,13 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   w.n_tiles = (n_tracks + SCAN_TILE - 1) / SCAN_TILE;
   w.n_chunks = (uint32_t)((n_att + CHUNK_WINDOW - 1) >> CHUNK_SHIFT);
   w.n_groups = (w.n_chunks + COL_GROUP - 1) / COL_GROUP;
+  w.n_sub = (uint32_t)((n_att + SUB_WINDOW - 1) >> SUB_SHIFT);
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
   w.o_err = take(ERR_WORDS * 4);
   w.o_tile_sum = take(((size_t)w.n_tiles + 1) * 4);
   w.o_off = take(((size_t)n_tracks + 1) * 4);
+  w.o_sub_first = take(((size_t)w.n_chunks * SUBS_PER_CHUNK + 2) * 4);
   w.o_len = take((size_t)LEN_BINS * 4 * 3);             // len_hist, len_base, len_cursor
   w.o_perm = take((size_t)n_tracks * 4);
   w.o_att_cnt = take((size_t)n_bins * 4);
@@ -112,14 +119,24 @@ int check_args(const tmd_ctx* ctx, const tmd_compressed* in, const tmd_output* o
   return TMD_OK;
 }
 
-#define TMD_LAUNCH_CHECK(name)                                                                  \
-  do {                                                                                          \
-    if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA;                                 \
-    if (timing && ctx->launches < TMD_MAX_KERNELS) {                                            \
-      ctx->kernel_names[ctx->launches] = name;                                                  \
-      if (cudaEventRecord(ctx->events[ctx->launches + 1], st) != cudaSuccess) return TMD_ERR_CUDA; \
-    }                                                                                           \
-    ctx->launches++;                                                                            \
+// Launch bookkeeping: TMD_BEFORE(stream) ... kernel<<<>>> ... TMD_AFTER(name, stream)
+#define TMD_BEFORE(stream)                                                                                  \
+  do {                                                                                                      \
+    if (timing && ctx->launches < TMD_MAX_KERNELS &&                                                        \
+        cudaEventRecord(ctx->ev_t0[ctx->launches], stream) != cudaSuccess) return TMD_ERR_CUDA;             \
+  } while (0)
+#define TMD_AFTER(name, stream)                                                                             \
+  do {                                                                                                      \
+    if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA;                                             \
+    if (timing && ctx->launches < TMD_MAX_KERNELS) {                                                        \
+      ctx->kernel_names[ctx->launches] = name;                                                              \
+      if (cudaEventRecord(ctx->ev_t1[ctx->launches], stream) != cudaSuccess) return TMD_ERR_CUDA;           \
+    }                                                                                                       \
+    ctx->launches++;                                                                                        \
+  } while (0)
+#define TMD_CUDA(call)                                   \
+  do {                                                   \
+    if ((call) != cudaSuccess) return TMD_ERR_CUDA;      \
   } while (0)
 
 }  // namespace
@@ -147,16 +164,25 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   cudaError_t e = cudaMalloc(&ctx->d_rows, sizeof(RowGeo) * g->n_rows);
   if (e == cudaSuccess) e = cudaMemcpy(ctx->d_rows, h, sizeof(RowGeo) * g->n_rows, cudaMemcpyHostToDevice);
   free(h);
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(CHUNK_WINDOW * 4 + (size_t)g->n_sectors_out * g->n_rows * 8));
+  const uint32_t n_bins_c = g->n_sectors_out * g->n_rows;
+  ctx->rank_smem = (((size_t)WR_GRANULES * 18 + 7) & ~(size_t)7) * 2 + (size_t)SUB_WINDOW * 2 + (size_t)n_bins_c * 8 +
+                   (size_t)(SUB_WINDOW / 32) * 8;
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_walk_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->rank_smem);
   ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_track_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
+  if (e == cudaSuccess) {
+    int lo = 0, hi = 0;   // numerically lowest = highest priority: the short integer kernels should not queue behind the decode
+    e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+    if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&ctx->side, cudaStreamNonBlocking, hi);
+  }
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_rel, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
   if (e != cudaSuccess) {
     cudaGetLastError();
-    if (ctx->d_rows) cudaFree(ctx->d_rows);
-    delete ctx;
+    tmd_destroy(ctx);
     return TMD_ERR_CUDA;
   }
   DevGeo& G = ctx->geo;
@@ -168,6 +194,8 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   volatile float qk = 0.0625f * kb;
   G.qk = qk;
   G.rows = ctx->d_rows;
+  G.rows_magic = (1u << 24) / g->n_rows + 1u;
+  G.az_magic = (1u << 24) / g->n_az + 1u;
   *out_ctx = ctx;
   return TMD_OK;
 }
@@ -203,91 +231,126 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
   uint2* d_inter = (uint2*)(ws + W.o_inter);
   const bool validate = (flags & TMD_VALIDATE) != 0, timing = (flags & TMD_TIMING) != 0;
+  uint32_t* d_subfirst = (uint32_t*)(ws + W.o_sub_first);
+  cudaStream_t s2 = (flags & TMD_SERIAL) ? st : ctx->side;   // TMD_SERIAL: one stream, kernels back to back
   ctx->launches = 0;
   ctx->timing_valid = false;
-  if (timing) {
-    if (!ctx->events_created) {
-      for (int i = 0; i <= TMD_MAX_KERNELS; ++i)
-        if (cudaEventCreate(&ctx->events[i]) != cudaSuccess) return TMD_ERR_CUDA;
-      ctx->events_created = true;
+  if (timing && !ctx->events_created) {
+    for (int i = 0; i < TMD_MAX_KERNELS; ++i) {
+      TMD_CUDA(cudaEventCreate(&ctx->ev_t0[i]));
+      TMD_CUDA(cudaEventCreate(&ctx->ev_t1[i]));
     }
-    if (cudaEventRecord(ctx->events[0], st) != cudaSuccess) return TMD_ERR_CUDA;
+    ctx->events_created = true;
   }
-  if (cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+  TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
 
-  if (n_trk > 0) {  // A1: track offsets + chunk table
+  if (n_trk > 0) {  // A1: track offsets; table of the first track of every sub-chunk window
+    TMD_BEFORE(st);
     k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile);
-    TMD_LAUNCH_CHECK("track_tile_sums");
+    TMD_AFTER("track_tile_sums", st);
+    TMD_BEFORE(st);
     k_scan_tile_sums<<<1, 1024, 0, st>>>(d_tile, W.n_tiles);
-    TMD_LAUNCH_CHECK("scan_tile_sums");
+    TMD_AFTER("scan_tile_sums", st);
+    TMD_BEFORE(st);
     k_track_offsets<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile, W.n_tiles, d_off);
-    TMD_LAUNCH_CHECK("track_offsets");
+    TMD_AFTER("track_offsets", st);
   }
   if (validate) {
+    TMD_BEFORE(st);
     k_validate<<<148, 256, 0, st>>>(G, *in, d_off, d_err);
-    TMD_LAUNCH_CHECK("validate");
+    TMD_AFTER("validate", st);
     uint32_t h_err[ERR_WORDS];
-    if (cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+    TMD_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
+    TMD_CUDA(cudaStreamSynchronize(st));
     if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;
   }
   if (n_trk > 0) {
-    // A2: load-balance order (counting sort by cluster count, longest first)
-    if (cudaMemsetAsync(d_len, 0, LEN_BINS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+    const uint32_t n_win = W.n_chunks * SUBS_PER_CHUNK;   // windows past n_attached get first = n_tracks
+    TMD_BEFORE(st);
+    k_window_table<<<(n_trk + 1 + 255) / 256, 256, 0, st>>>(d_off, n_trk, d_subfirst, n_win, SUB_SHIFT);
+    TMD_AFTER("window_table", st);
+  }
+  if (n_trk > 0) {  // A2: load-balance order (counting sort by cluster count, longest first)
+    TMD_CUDA(cudaMemsetAsync(d_len, 0, LEN_BINS * 4, st));
     const uint32_t sort_blocks = (n_trk + SORT_TILE - 1) / SORT_TILE;
+    TMD_BEFORE(st);
     k_len_hist<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len);
-    TMD_LAUNCH_CHECK("len_hist");
+    TMD_AFTER("len_hist", st);
+    TMD_BEFORE(st);
     k_len_scan<<<1, 1024, 0, st>>>(d_len, d_len + LEN_BINS, d_len + 2 * LEN_BINS);
-    TMD_LAUNCH_CHECK("len_scan");
+    TMD_AFTER("len_scan", st);
+    TMD_BEFORE(st);
     k_len_perm<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len + LEN_BINS, d_len + 2 * LEN_BINS, d_perm);
-    TMD_LAUNCH_CHECK("len_perm");
-    // A3 (walk) + A5: track-model decode -> intermediate records in g order
-    DecodeArgs D;
-    D.off = d_off; D.perm = d_perm; D.in = *in; D.inter = d_inter;
-    D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
-    k_track_decode<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
-    TMD_LAUNCH_CHECK("track_decode");
-    // A3 (count): per-chunk histogram + ranks
-    RankArgs R;
-    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att;
-    const size_t rank_smem = CHUNK_WINDOW * 4 + (size_t)n_bins * 8;
-    k_rank<<<W.n_chunks, RANK_THREADS, rank_smem, st>>>(G, R);
-    TMD_LAUNCH_CHECK("rank");
+    TMD_AFTER("len_perm", st);
+  }
+  // ---- fork: the integer side (A3 walk + ranks, A4, A7) on the context's second stream
+  TMD_CUDA(cudaEventRecord(ctx->ev_fork, st));
+  TMD_CUDA(cudaStreamWaitEvent(s2, ctx->ev_fork, 0));
+  if (n_trk > 0) {
+    WalkRankArgs R;
+    R.off = d_off; R.sub_first = d_subfirst; R.trk_row0 = in->trk_row0; R.trk_sec0 = in->trk_sec0;
+    R.a_rowdiff = in->a_rowdiff; R.a_secleg = in->a_secleg; R.hist = d_hist; R.rank16 = d_rank;
+    R.n_tracks = n_trk; R.n_attached = n_att; R.n_chunks = W.n_chunks;
+    const uint32_t want_blocks = 2u * (uint32_t)ctx->n_sm;
+    R.chunks_per_block = (W.n_chunks + want_blocks - 1) / want_blocks;
+    const uint32_t rank_blocks = (W.n_chunks + R.chunks_per_block - 1) / R.chunks_per_block;
+    TMD_BEFORE(s2);
+    k_walk_rank<<<rank_blocks, WR_THREADS, ctx->rank_smem, s2>>>(G, R);
+    TMD_AFTER("walk_rank", s2);
     // A4: column scan over chunks
     dim3 cg((n_bins + 255) / 256, W.n_groups);
-    k_col_group_sums<<<cg, 256, 0, st>>>(d_hist, W.n_chunks, n_bins, d_gsum);
-    TMD_LAUNCH_CHECK("col_group_sums");
-    k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, st>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
-    TMD_LAUNCH_CHECK("col_group_scan");
+    TMD_BEFORE(s2);
+    k_col_group_sums<<<cg, 256, 0, s2>>>(d_hist, W.n_chunks, n_bins, d_gsum);
+    TMD_AFTER("col_group_sums", s2);
+    TMD_BEFORE(s2);
+    k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, s2>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
+    TMD_AFTER("col_group_scan", s2);
   } else {
-    if (cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
+    TMD_CUDA(cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, s2));
   }
-  k_bin_offsets<<<1, 1024, 0, st>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
-  TMD_LAUNCH_CHECK("bin_offsets");
+  TMD_BEFORE(s2);
+  k_bin_offsets<<<1, 1024, 0, s2>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
+  TMD_AFTER("bin_offsets", s2);
   if (n_trk > 0) {
     dim3 cg((n_bins + 255) / 256, W.n_groups);
-    k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
-    TMD_LAUNCH_CHECK("col_apply");
-    // A6: copy-through + scatter
-    ScatterArgs S;
-    S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
-    S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
-    S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un;
-    k_scatter<<<(n_att + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, 0, st>>>(G, S);
-    TMD_LAUNCH_CHECK("scatter");
+    TMD_BEFORE(s2);
+    k_col_apply<<<cg, 256, 0, s2>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
+    TMD_AFTER("col_apply", s2);
+    TMD_CUDA(cudaEventRecord(ctx->ev_rel, s2));
   }
   if (n_un > 0) {  // A7
     UnattachedArgs U;
     U.in = *in; U.u_start = d_ustart; U.bin_offset = out->bin_offset; U.att_cnt = d_attcnt;
     U.clusters = (uint4*)out->clusters; U.n_clusters_total = n_att + n_un;
-    k_unattached<<<n_bins, UNATT_THREADS, 0, st>>>(G, U);
-    TMD_LAUNCH_CHECK("unattached");
+    TMD_BEFORE(s2);
+    k_unattached<<<n_bins, UNATT_THREADS, 0, s2>>>(G, U);
+    TMD_AFTER("unattached", s2);
   }
+  TMD_CUDA(cudaEventRecord(ctx->ev_join, s2));
+  // ---- the caller's stream: A5 track-model decode, then (after the ranks) A6 scatter
+  if (n_trk > 0) {
+    DecodeArgs D;
+    D.off = d_off; D.perm = d_perm; D.in = *in; D.inter = d_inter;
+    D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
+    TMD_BEFORE(st);
+    k_track_decode<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
+    TMD_AFTER("track_decode", st);
+    TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_rel, 0));
+    ScatterArgs S;
+    S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
+    S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
+    S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un;
+    const uint32_t per_block = SCATTER_THREADS * SCATTER_VEC;
+    TMD_BEFORE(st);
+    k_scatter<<<(n_att + per_block - 1) / per_block, SCATTER_THREADS, 0, st>>>(G, S);
+    TMD_AFTER("scatter", st);
+  }
+  TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));   // join: everything is ordered before later work on `st`
   ctx->timing_valid = timing;
   if (validate) {
     uint32_t h_err[ERR_WORDS];
-    if (cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+    TMD_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
+    TMD_CUDA(cudaStreamSynchronize(st));
     if (h_err[ERR_TRACK_FIELD] || h_err[ERR_SECTOR_OUT]) return TMD_ERR_CORRUPT;
   }
   return TMD_OK;
@@ -297,11 +360,11 @@ int tmd_kernel_times(tmd_ctx* ctx, int max_kernels, const char** names, float* m
   if (!ctx || !names || !ms || max_kernels < 0) return TMD_ERR_ARG;
   if (!ctx->timing_valid) return 0;
   const int n = ctx->launches < TMD_MAX_KERNELS ? ctx->launches : TMD_MAX_KERNELS;
-  if (n > 0 && cudaEventSynchronize(ctx->events[n]) != cudaSuccess) return TMD_ERR_CUDA;
   int k = 0;
   for (; k < n && k < max_kernels; ++k) {
     names[k] = ctx->kernel_names[k];
-    if (cudaEventElapsedTime(&ms[k], ctx->events[k], ctx->events[k + 1]) != cudaSuccess) return TMD_ERR_CUDA;
+    if (cudaEventSynchronize(ctx->ev_t1[k]) != cudaSuccess) return TMD_ERR_CUDA;
+    if (cudaEventElapsedTime(&ms[k], ctx->ev_t0[k], ctx->ev_t1[k]) != cudaSuccess) return TMD_ERR_CUDA;
   }
   return k;
 }
@@ -410,10 +473,14 @@ int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uin
 
 int tmd_destroy(tmd_ctx* ctx) {
   if (!ctx) return TMD_OK;
+  if (ctx->side) { cudaStreamSynchronize(ctx->side); cudaStreamDestroy(ctx->side); }
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->ev_rel) cudaEventDestroy(ctx->ev_rel);
+  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->d_rows) cudaFree(ctx->d_rows);
   if (ctx->events_created)
-    for (int i = 0; i <= TMD_MAX_KERNELS; ++i) cudaEventDestroy(ctx->events[i]);
+    for (int i = 0; i < TMD_MAX_KERNELS; ++i) { cudaEventDestroy(ctx->ev_t0[i]); cudaEventDestroy(ctx->ev_t1[i]); }
   delete ctx;
   return TMD_OK;
 }

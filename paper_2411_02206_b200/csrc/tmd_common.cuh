@@ -16,7 +16,6 @@ namespace tmd {
 // bins, a column scan over chunks, and ranks inside the chunk.
 constexpr int CHUNK_SHIFT = 15;
 constexpr uint32_t CHUNK_WINDOW = 1u << CHUNK_SHIFT;
-constexpr uint32_t RANK_CAP = 36864;    // clusters of a chunk that the shared-memory rank path can hold
 constexpr uint32_t MAX_BINS = 8192;     // n_sectors_out * n_rows
 constexpr uint32_t COL_GROUP = 64;      // chunks per group in the column scan
 constexpr uint16_t BIN_INVALID = 0xFFFFu;
@@ -29,6 +28,8 @@ struct DevGeo {
   uint32_t n_az, n_sides, n_sectors_out, n_rows, n_bins;
   float cos_a, sin_a;
   float qk;             // fmul(0.0625f, fmul(bz_tesla, 0.00299792458f))
+  uint32_t rows_magic;  // floor(2^24 / n_rows) + 1:  bin / n_rows == (bin * rows_magic) >> 24  for bin < 8192 (< 2^24 / n_rows)
+  uint32_t az_magic;    // floor(2^24 / n_az) + 1, same trick for values < 64
   const RowGeo* rows;   // DEVICE [n_rows]
 };
 

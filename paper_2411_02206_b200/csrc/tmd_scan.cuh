@@ -91,17 +91,17 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_track_offsets(const uint16_t* 
   if (blockIdx.x == n_tiles - 1 && threadIdx.x == 0) off[n_tracks] = tile_sum[n_tiles];
 }
 
-// Chunk table: chunk c = the tracks t with (off[t] >> CHUNK_SHIFT) == c = [chunk_first[c], chunk_first[c+1]).
-// chunk_first[c] = first track with off[t] >= c << CHUNK_SHIFT; off is strictly increasing (trk_ncl >= 1), so track t
-// is that first track for every c with off[t-1] < c*W <= off[t].  One thread per t in [0, n_tracks].
-__global__ void k_chunk_table(const uint32_t* __restrict__ off, uint32_t n_tracks, uint32_t* __restrict__ chunk_first,
-                              uint32_t n_chunks) {
+// Window table: first[c] = first track t with off[t] >= c << shift (off is strictly increasing because trk_ncl >= 1), so
+// the tracks whose first cluster lies in window c are [first[c], first[c+1]); first[n_windows] = n_tracks.
+// Track t is that first track for every c with off[t-1] < c << shift <= off[t].  One thread per t in [0, n_tracks].
+__global__ void k_window_table(const uint32_t* __restrict__ off, uint32_t n_tracks, uint32_t* __restrict__ first,
+                               uint32_t n_windows, uint32_t shift) {
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t > n_tracks) return;
-  const uint32_t c_lo = (t == 0) ? 0 : (off[t - 1] >> CHUNK_SHIFT) + 1;
-  uint32_t c_hi = (t == n_tracks) ? n_chunks : (off[t] >> CHUNK_SHIFT);
-  if (c_hi > n_chunks) c_hi = n_chunks;  // malformed counts must not write out of bounds
-  for (uint32_t c = c_lo; c <= c_hi; ++c) chunk_first[c] = t;
+  const uint32_t c_lo = (t == 0) ? 0 : (off[t - 1] >> shift) + 1;
+  uint32_t c_hi = (t == n_tracks) ? n_windows : (off[t] >> shift);
+  if (c_hi > n_windows) c_hi = n_windows;  // malformed counts must not write out of bounds
+  for (uint32_t c = c_lo; c <= c_hi; ++c) first[c] = t;
 }
 
 // ---- A4 part 1: column sums over groups of chunks ---------------------------------------------------------------------

@@ -18,7 +18,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT = 0, -1, -2, -3, -4, -5
 TMD_VALIDATE = 1
 TMD_TIMING = 2
-TMD_MAX_KERNELS = 16
+TMD_SERIAL = 4
+TMD_MAX_KERNELS = 24
 PROBE_FINAL = 0xFFFFFFFF
 
 # (field name, numpy dtype) in the order of struct tmd_compressed
