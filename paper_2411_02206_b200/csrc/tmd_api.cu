@@ -20,10 +20,10 @@ struct tmd_ctx {
   RowGeo* d_rows;
   int device;
   int launches;
-  // Second stream of tmd_decode: the integer side of the path (walk + ranks, column scan, bin offsets, unattached
-  // clusters) runs there, concurrently with the floating-point track decode on the caller's stream.
+  // Second stream of tmd_decode: the unattached clusters (A7) are decoded there while the attached ones are scattered
+  // (A6) on the caller's stream.
   cudaStream_t side;
-  cudaEvent_t ev_fork, ev_rel, ev_join;
+  cudaEvent_t ev_fork, ev_join;
   // TMD_TIMING: one event pair around every kernel of the last tmd_decode, recorded on the stream it ran on
   cudaEvent_t ev_t0[TMD_MAX_KERNELS], ev_t1[TMD_MAX_KERNELS];
   const char* kernel_names[TMD_MAX_KERNELS];
@@ -41,8 +41,8 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
 struct Workspace {
-  uint32_t n_tiles, n_chunks, n_groups, n_sub;
-  size_t o_err, o_tile_sum, o_off, o_sub_first, o_len, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
+  uint32_t n_tiles, n_chunks, n_groups;
+  size_t o_err, o_tile_sum, o_off, o_len, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
 };
 
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
@@ -50,13 +50,11 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   w.n_tiles = (n_tracks + SCAN_TILE - 1) / SCAN_TILE;
   w.n_chunks = (uint32_t)((n_att + CHUNK_WINDOW - 1) >> CHUNK_SHIFT);
   w.n_groups = (w.n_chunks + COL_GROUP - 1) / COL_GROUP;
-  w.n_sub = (uint32_t)((n_att + SUB_WINDOW - 1) >> SUB_SHIFT);
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
   w.o_err = take(ERR_WORDS * 4);
   w.o_tile_sum = take(((size_t)w.n_tiles + 1) * 4);
   w.o_off = take(((size_t)n_tracks + 1) * 4);
-  w.o_sub_first = take(((size_t)w.n_chunks * SUBS_PER_CHUNK + 2) * 4);
   w.o_len = take((size_t)LEN_BINS * 4 * 3);             // len_hist, len_base, len_cursor
   w.o_perm = take((size_t)n_tracks * 4);
   w.o_att_cnt = take((size_t)n_bins * 4);
@@ -165,9 +163,8 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   if (e == cudaSuccess) e = cudaMemcpy(ctx->d_rows, h, sizeof(RowGeo) * g->n_rows, cudaMemcpyHostToDevice);
   free(h);
   const uint32_t n_bins_c = g->n_sectors_out * g->n_rows;
-  ctx->rank_smem = (((size_t)WR_GRANULES * 18 + 7) & ~(size_t)7) * 2 + (size_t)SUB_WINDOW * 2 + (size_t)n_bins_c * 8 +
-                   (size_t)(SUB_WINDOW / 32) * 8;
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_walk_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->rank_smem);
+  ctx->rank_smem = (size_t)WR_WARPS * wr_warp_smem(n_bins_c);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->rank_smem);
   ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_track_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
@@ -178,7 +175,6 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
     if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&ctx->side, cudaStreamNonBlocking, hi);
   }
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_rel, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
   if (e != cudaSuccess) {
     cudaGetLastError();
@@ -195,7 +191,6 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   G.qk = qk;
   G.rows = ctx->d_rows;
   G.rows_magic = (1u << 24) / g->n_rows + 1u;
-  G.az_magic = (1u << 24) / g->n_az + 1u;
   *out_ctx = ctx;
   return TMD_OK;
 }
@@ -231,7 +226,6 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
   uint2* d_inter = (uint2*)(ws + W.o_inter);
   const bool validate = (flags & TMD_VALIDATE) != 0, timing = (flags & TMD_TIMING) != 0;
-  uint32_t* d_subfirst = (uint32_t*)(ws + W.o_sub_first);
   cudaStream_t s2 = (flags & TMD_SERIAL) ? st : ctx->side;   // TMD_SERIAL: one stream, kernels back to back
   ctx->launches = 0;
   ctx->timing_valid = false;
@@ -244,7 +238,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   }
   TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
 
-  if (n_trk > 0) {  // A1: track offsets; table of the first track of every sub-chunk window
+  if (n_trk > 0) {  // A1: track offsets
     TMD_BEFORE(st);
     k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile);
     TMD_AFTER("track_tile_sums", st);
@@ -265,12 +259,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;
   }
   if (n_trk > 0) {
-    const uint32_t n_win = W.n_chunks * SUBS_PER_CHUNK;   // windows past n_attached get first = n_tracks
-    TMD_BEFORE(st);
-    k_window_table<<<(n_trk + 1 + 255) / 256, 256, 0, st>>>(d_off, n_trk, d_subfirst, n_win, SUB_SHIFT);
-    TMD_AFTER("window_table", st);
-  }
-  if (n_trk > 0) {  // A2: load-balance order (counting sort by cluster count, longest first)
+    // A2: load-balance order (counting sort by cluster count, longest first)
     TMD_CUDA(cudaMemsetAsync(d_len, 0, LEN_BINS * 4, st));
     const uint32_t sort_blocks = (n_trk + SORT_TILE - 1) / SORT_TILE;
     TMD_BEFORE(st);
@@ -282,60 +271,60 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     TMD_BEFORE(st);
     k_len_perm<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len + LEN_BINS, d_len + 2 * LEN_BINS, d_perm);
     TMD_AFTER("len_perm", st);
-  }
-  // ---- fork: the integer side (A3 walk + ranks, A4, A7) on the context's second stream
-  TMD_CUDA(cudaEventRecord(ctx->ev_fork, st));
-  TMD_CUDA(cudaStreamWaitEvent(s2, ctx->ev_fork, 0));
-  if (n_trk > 0) {
-    WalkRankArgs R;
-    R.off = d_off; R.sub_first = d_subfirst; R.trk_row0 = in->trk_row0; R.trk_sec0 = in->trk_sec0;
-    R.a_rowdiff = in->a_rowdiff; R.a_secleg = in->a_secleg; R.hist = d_hist; R.rank16 = d_rank;
-    R.n_tracks = n_trk; R.n_attached = n_att; R.n_chunks = W.n_chunks;
-    const uint32_t want_blocks = 2u * (uint32_t)ctx->n_sm;
-    R.chunks_per_block = (W.n_chunks + want_blocks - 1) / want_blocks;
-    const uint32_t rank_blocks = (W.n_chunks + R.chunks_per_block - 1) / R.chunks_per_block;
-    TMD_BEFORE(s2);
-    k_walk_rank<<<rank_blocks, WR_THREADS, ctx->rank_smem, s2>>>(G, R);
-    TMD_AFTER("walk_rank", s2);
-    // A4: column scan over chunks
-    dim3 cg((n_bins + 255) / 256, W.n_groups);
-    TMD_BEFORE(s2);
-    k_col_group_sums<<<cg, 256, 0, s2>>>(d_hist, W.n_chunks, n_bins, d_gsum);
-    TMD_AFTER("col_group_sums", s2);
-    TMD_BEFORE(s2);
-    k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, s2>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
-    TMD_AFTER("col_group_scan", s2);
-  } else {
-    TMD_CUDA(cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, s2));
-  }
-  TMD_BEFORE(s2);
-  k_bin_offsets<<<1, 1024, 0, s2>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
-  TMD_AFTER("bin_offsets", s2);
-  if (n_trk > 0) {
-    dim3 cg((n_bins + 255) / 256, W.n_groups);
-    TMD_BEFORE(s2);
-    k_col_apply<<<cg, 256, 0, s2>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
-    TMD_AFTER("col_apply", s2);
-    TMD_CUDA(cudaEventRecord(ctx->ev_rel, s2));
-  }
-  if (n_un > 0) {  // A7
-    UnattachedArgs U;
-    U.in = *in; U.u_start = d_ustart; U.bin_offset = out->bin_offset; U.att_cnt = d_attcnt;
-    U.clusters = (uint4*)out->clusters; U.n_clusters_total = n_att + n_un;
-    TMD_BEFORE(s2);
-    k_unattached<<<n_bins, UNATT_THREADS, 0, s2>>>(G, U);
-    TMD_AFTER("unattached", s2);
-  }
-  TMD_CUDA(cudaEventRecord(ctx->ev_join, s2));
-  // ---- the caller's stream: A5 track-model decode, then (after the ranks) A6 scatter
-  if (n_trk > 0) {
+    // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
     DecodeArgs D;
     D.off = d_off; D.perm = d_perm; D.in = *in; D.inter = d_inter;
     D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
     TMD_BEFORE(st);
     k_track_decode<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
     TMD_AFTER("track_decode", st);
-    TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_rel, 0));
+    // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
+    RankArgs R;
+    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att; R.n_chunks = W.n_chunks;
+    uint32_t per_sm = (uint32_t)((size_t)(227 * 1024) / (ctx->rank_smem + 1024));
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 16) per_sm = 16;
+    uint32_t rank_blocks = (W.n_chunks + WR_WARPS - 1) / WR_WARPS;
+    if (rank_blocks > per_sm * (uint32_t)ctx->n_sm) rank_blocks = per_sm * (uint32_t)ctx->n_sm;
+    TMD_BEFORE(st);
+    k_rank<<<rank_blocks, WR_THREADS, ctx->rank_smem, st>>>(G, R);
+    TMD_AFTER("rank", st);
+    // A4: column scan over chunks
+    dim3 cg((n_bins + 255) / 256, W.n_groups);
+    TMD_BEFORE(st);
+    k_col_group_sums<<<cg, 256, 0, st>>>(d_hist, W.n_chunks, n_bins, d_gsum);
+    TMD_AFTER("col_group_sums", st);
+    TMD_BEFORE(st);
+    k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, st>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
+    TMD_AFTER("col_group_scan", st);
+  } else {
+    TMD_CUDA(cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, st));
+  }
+  TMD_BEFORE(st);
+  k_bin_offsets<<<1, 1024, 0, st>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
+  TMD_AFTER("bin_offsets", st);
+  // ---- fork: A7 (unattached clusters) on the context's second stream, next to A6 on the caller's
+  const bool fork = n_un > 0 && n_trk > 0 && s2 != st;
+  if (n_un > 0) {
+    cudaStream_t su = fork ? s2 : st;
+    if (fork) {
+      TMD_CUDA(cudaEventRecord(ctx->ev_fork, st));
+      TMD_CUDA(cudaStreamWaitEvent(s2, ctx->ev_fork, 0));
+    }
+    UnattachedArgs U;
+    U.in = *in; U.u_start = d_ustart; U.bin_offset = out->bin_offset; U.att_cnt = d_attcnt;
+    U.clusters = (uint4*)out->clusters; U.n_clusters_total = n_att + n_un;
+    TMD_BEFORE(su);
+    k_unattached<<<n_bins, UNATT_THREADS, 0, su>>>(G, U);
+    TMD_AFTER("unattached", su);
+    if (fork) TMD_CUDA(cudaEventRecord(ctx->ev_join, s2));
+  }
+  if (n_trk > 0) {
+    dim3 cg((n_bins + 255) / 256, W.n_groups);
+    TMD_BEFORE(st);
+    k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
+    TMD_AFTER("col_apply", st);
+    // A6: copy-through + scatter
     ScatterArgs S;
     S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
     S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
@@ -345,7 +334,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     k_scatter<<<(n_att + per_block - 1) / per_block, SCATTER_THREADS, 0, st>>>(G, S);
     TMD_AFTER("scatter", st);
   }
-  TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));   // join: everything is ordered before later work on `st`
+  if (fork) TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));   // join: everything is ordered before later work on `st`
   ctx->timing_valid = timing;
   if (validate) {
     uint32_t h_err[ERR_WORDS];
@@ -475,7 +464,6 @@ int tmd_destroy(tmd_ctx* ctx) {
   if (!ctx) return TMD_OK;
   if (ctx->side) { cudaStreamSynchronize(ctx->side); cudaStreamDestroy(ctx->side); }
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-  if (ctx->ev_rel) cudaEventDestroy(ctx->ev_rel);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->arena) cudaFree(ctx->arena);
   if (ctx->d_rows) cudaFree(ctx->d_rows);

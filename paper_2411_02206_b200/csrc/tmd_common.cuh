@@ -29,7 +29,6 @@ struct DevGeo {
   float cos_a, sin_a;
   float qk;             // fmul(0.0625f, fmul(bz_tesla, 0.00299792458f))
   uint32_t rows_magic;  // floor(2^24 / n_rows) + 1:  bin / n_rows == (bin * rows_magic) >> 24  for bin < 8192 (< 2^24 / n_rows)
-  uint32_t az_magic;    // floor(2^24 / n_az) + 1, same trick for values < 64
   const RowGeo* rows;   // DEVICE [n_rows]
 };
 
@@ -58,6 +57,15 @@ __device__ __forceinline__ uint32_t walk_step(WalkState& w, uint32_t rowdiff, ui
   w.az = a >= n_az ? a - n_az : a;
   return d;
 }
+
+// cp.async (LDGSTS): 16-byte global -> shared copy; bytes past src_bytes are zero-filled
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src, uint32_t src_bytes) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gmem_src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
 

@@ -91,19 +91,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_track_offsets(const uint16_t* 
   if (blockIdx.x == n_tiles - 1 && threadIdx.x == 0) off[n_tracks] = tile_sum[n_tiles];
 }
 
-// Window table: first[c] = first track t with off[t] >= c << shift (off is strictly increasing because trk_ncl >= 1), so
-// the tracks whose first cluster lies in window c are [first[c], first[c+1]); first[n_windows] = n_tracks.
-// Track t is that first track for every c with off[t-1] < c << shift <= off[t].  One thread per t in [0, n_tracks].
-__global__ void k_window_table(const uint32_t* __restrict__ off, uint32_t n_tracks, uint32_t* __restrict__ first,
-                               uint32_t n_windows, uint32_t shift) {
-  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t > n_tracks) return;
-  const uint32_t c_lo = (t == 0) ? 0 : (off[t - 1] >> shift) + 1;
-  uint32_t c_hi = (t == n_tracks) ? n_windows : (off[t] >> shift);
-  if (c_hi > n_windows) c_hi = n_windows;  // malformed counts must not write out of bounds
-  for (uint32_t c = c_lo; c <= c_hi; ++c) first[c] = t;
-}
-
 // ---- A4 part 1: column sums over groups of chunks ---------------------------------------------------------------------
 // hist[c][b] (u16) = attached clusters of chunk c in bin b.   gsum[grp][b] = sum over the group's chunks.
 __global__ void __launch_bounds__(256) k_col_group_sums(const uint16_t* __restrict__ hist, uint32_t n_chunks, uint32_t n_bins,
