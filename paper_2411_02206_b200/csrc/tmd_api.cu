@@ -42,7 +42,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
 struct Workspace {
   uint32_t n_tiles, n_chunks, n_groups;
-  size_t o_err, o_tile_sum, o_off, o_len, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
+  size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
 };
 
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
@@ -55,7 +55,6 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   w.o_err = take(ERR_WORDS * 4);
   w.o_tile_sum = take(((size_t)w.n_tiles + 1) * 4);
   w.o_off = take(((size_t)n_tracks + 1) * 4);
-  w.o_len = take((size_t)LEN_BINS * 4 * 3);             // len_hist, len_base, len_cursor
   w.o_perm = take((size_t)n_tracks * 4);
   w.o_att_cnt = take((size_t)n_bins * 4);
   w.o_u_start = take(((size_t)n_bins + 1) * 4);
@@ -191,6 +190,7 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   G.qk = qk;
   G.rows = ctx->d_rows;
   G.rows_magic = (1u << 24) / g->n_rows + 1u;
+  G.az_magic = (1u << 24) / g->n_az + 1u;
   *out_ctx = ctx;
   return TMD_OK;
 }
@@ -216,7 +216,6 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   uint32_t* d_err = (uint32_t*)(ws + W.o_err);
   uint32_t* d_tile = (uint32_t*)(ws + W.o_tile_sum);
   uint32_t* d_off = (uint32_t*)(ws + W.o_off);
-  uint32_t* d_len = (uint32_t*)(ws + W.o_len);
   uint32_t* d_perm = (uint32_t*)(ws + W.o_perm);
   uint32_t* d_attcnt = (uint32_t*)(ws + W.o_att_cnt);
   uint32_t* d_ustart = (uint32_t*)(ws + W.o_u_start);
@@ -259,24 +258,17 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;
   }
   if (n_trk > 0) {
-    // A2: load-balance order (counting sort by cluster count, longest first)
-    TMD_CUDA(cudaMemsetAsync(d_len, 0, LEN_BINS * 4, st));
-    const uint32_t sort_blocks = (n_trk + SORT_TILE - 1) / SORT_TILE;
+    // A2: load-balance order (counting sort by cluster count, longest first, inside windows of consecutive tracks)
     TMD_BEFORE(st);
-    k_len_hist<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len);
-    TMD_AFTER("len_hist", st);
-    TMD_BEFORE(st);
-    k_len_scan<<<1, 1024, 0, st>>>(d_len, d_len + LEN_BINS, d_len + 2 * LEN_BINS);
-    TMD_AFTER("len_scan", st);
-    TMD_BEFORE(st);
-    k_len_perm<<<sort_blocks, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_len + LEN_BINS, d_len + 2 * LEN_BINS, d_perm);
-    TMD_AFTER("len_perm", st);
+    k_len_sort_window<<<(n_trk + SORT_WINDOW - 1) / SORT_WINDOW, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_perm);
+    TMD_AFTER("len_sort_window", st);
     // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
     DecodeArgs D;
     D.off = d_off; D.perm = d_perm; D.in = *in; D.inter = d_inter;
     D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
     TMD_BEFORE(st);
-    k_track_decode<<<(n_trk + DECODE_THREADS - 1) / DECODE_THREADS, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
+    const uint32_t decode_blocks = (n_trk + DECODE_THREADS - 1) / DECODE_THREADS;
+    k_track_decode<<<decode_blocks, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
     TMD_AFTER("track_decode", st);
     // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
     RankArgs R;
@@ -329,9 +321,8 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
     S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
     S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un;
-    const uint32_t per_block = SCATTER_THREADS * SCATTER_VEC;
     TMD_BEFORE(st);
-    k_scatter<<<(n_att + per_block - 1) / per_block, SCATTER_THREADS, 0, st>>>(G, S);
+    k_scatter<<<(n_att + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, 0, st>>>(G, S);
     TMD_AFTER("scatter", st);
   }
   if (fork) TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));   // join: everything is ordered before later work on `st`

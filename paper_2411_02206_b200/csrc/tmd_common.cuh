@@ -29,6 +29,7 @@ struct DevGeo {
   float cos_a, sin_a;
   float qk;             // fmul(0.0625f, fmul(bz_tesla, 0.00299792458f))
   uint32_t rows_magic;  // floor(2^24 / n_rows) + 1:  bin / n_rows == (bin * rows_magic) >> 24  for bin < 8192 (< 2^24 / n_rows)
+  uint32_t az_magic;    // floor(2^24 / n_az) + 1, the same for values < 64
   const RowGeo* rows;   // DEVICE [n_rows]
 };
 
