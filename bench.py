@@ -51,7 +51,7 @@ def kernel_algorithmic_bytes(n_trk: int, n_att: int, n_un: int, n_bins: int) -> 
 
 
 # ------------------------------------------------------------------------------------------------ workload on the device
-def build_workload(name: str, device, seed_offset: int = 0):
+def build_workload(name: str, device, seed_offset: int = 0, keep_truth: bool = False):
     """Synthetic time frame `name` (tmd_inputs.timeframe.WORKLOADS) as device tensors of the compressed SoA.
     Attached clusters: helix truth -> the library's own encoder (tmd_encode_attached); unattached: compressed domain."""
     import torch
@@ -78,41 +78,40 @@ def build_workload(name: str, device, seed_offset: int = 0):
     T.tmd_encode_attached(ctx, truth.trk_ncl, truth.trk_qptf, truth.att, truth.leg, arrays, ws,
                           torch.cuda.current_stream().cuda_stream)
     T.tmd_destroy(ctx)
-    del truth, ws
+    del ws
+    if not keep_truth:
+        truth = None
     arrays.update(tf.generate_unattached(geo, n_un, cfg.seed, device, "inv_x", single))
     torch.cuda.empty_cache()
-    return geo, arrays
+    return (geo, arrays, truth) if keep_truth else (geo, arrays)
 
 
-def sub_frame(arrays: dict, n_bins: int, n_trk_s: int, frac_un: float):
-    """A bounded sample of the workload as host numpy arrays: the first n_trk_s tracks with all their clusters and the
-    first floor(frac_un * count) unattached clusters of every bin (index selection only)."""
+def oracle_sample(workload: str, n_s: int, device):
+    """A bounded sample of `workload` for the CPU oracle: the first n_s tracks of the same generator recipe (same pT / length /
+    looper mix) and the same fraction of the unattached clusters.  The attached clusters are ENCODED BY THE ORACLE'S OWN
+    ENCODER -- nothing the oracle reads comes from the CUDA path."""
     import torch
+    from tmd_inputs import build_geometry, physical as ph, timeframe as tf
     from tmd_inputs.layout import COMPRESSED_FIELDS, Compressed
-    ncl = (arrays["trk_ncl"][:n_trk_s].to(torch.int64)) & 0xFFFF
-    n_att_s = int(ncl.sum())
-    cnt = arrays["u_bin_count"].to(torch.int64)
-    cnt_s = torch.floor(cnt.to(torch.float64) * frac_un).to(torch.int64)
-    start = torch.cumsum(cnt, 0) - cnt
-    start_s = torch.cumsum(cnt_s, 0) - cnt_s
-    n_un_s = int(cnt_s.sum())
-    bins = torch.repeat_interleave(torch.arange(n_bins, device=cnt.device), cnt_s)
-    idx = start[bins] + (torch.arange(n_un_s, device=cnt.device) - start_s[bins])
-    c = Compressed.empty(n_trk_s, n_att_s, n_un_s, n_bins)
-    for k, (dt, which) in COMPRESSED_FIELDS.items():
-        a = arrays[k]
-        if which == "n_tracks":
-            a = a[:n_trk_s]
-        elif which == "n_attached":
-            a = a[:n_att_s]
-        elif which == "n_residuals":
-            a = a[: n_att_s - n_trk_s]
-        elif which == "n_unattached":
-            a = a[idx]
-        else:
-            a = cnt_s.to(torch.int32)
-        getattr(c, k)[:] = a.cpu().numpy().view(np.dtype(dt))
-    return c
+    from oracle import tmd_oracle as O
+
+    geo = build_geometry(36)
+    mk, n_un, single = tf.WORKLOADS[workload]
+    cfg = mk()
+    n_s = min(cfg.n_tracks, n_s)
+    frac = n_s / cfg.n_tracks
+    cfg.n_tracks = n_s
+    tr = tf.generate_truth(cfg, geo, device, batch=400_000)
+    ev_att = tr.att.cpu().numpy().view(ph.CLUSTER_DTYPE).reshape(-1)
+    comp = O.encode(geo, BZ, tr.trk_ncl.cpu().numpy().view(np.uint16), tr.trk_qptf.cpu().numpy(), ev_att, tr.leg.cpu().numpy(),
+                    np.zeros(0, ph.CLUSTER_DTYPE))
+    del tr, ev_att
+    u = tf.generate_unattached(geo, int(n_un * frac), cfg.seed, device, "inv_x", single)
+    full = Compressed.empty(comp.n_tracks, comp.n_attached, int(u["u_qtot"].shape[0]), geo.n_bins)
+    for k, (dt, _) in COMPRESSED_FIELDS.items():
+        src = u[k].cpu().numpy().view(np.dtype(dt)) if k in u else getattr(comp, k)
+        getattr(full, k)[:] = src
+    return geo, full, n_s
 
 
 def time_oracle(geo, comp) -> float:
@@ -122,20 +121,15 @@ def time_oracle(geo, comp) -> float:
     return time.perf_counter() - t0
 
 
-def cpu_baseline(geo, arrays, n_trk: int, target_s: float = 12.0) -> dict:
-    """The oracle as it stands (single thread) on a bounded sample: calibrate on a small sample, then ~target_s of work."""
-    probe_trk = max(1, min(n_trk, 2000))
-    c = sub_frame(arrays, geo.n_bins, probe_trk, probe_trk / n_trk)
-    dt = max(time_oracle(geo, c), 1e-4)
-    rate = (c.n_attached + c.n_unattached) / dt
-    frac = min(1.0, target_s * rate / (int(arrays["a_qtot"].shape[0]) + int(arrays["u_qtot"].shape[0])))
-    n_s = max(probe_trk, int(n_trk * frac))
-    c = sub_frame(arrays, geo.n_bins, n_s, n_s / n_trk)
-    dt = time_oracle(geo, c)
-    n_cl = c.n_attached + c.n_unattached
+def cpu_baseline(workload: str, n_s: int, device) -> dict:
+    """The oracle as it stands (single thread) timed on a bounded sample of the workload (about 10 s of decoding at c3)."""
+    geo, comp, n_s = oracle_sample(workload, n_s, device)
+    dt = time_oracle(geo, comp)
+    n_cl = comp.n_attached + comp.n_unattached
     return {"value": n_cl / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"first {n_s} of {n_trk} tracks ({c.n_attached} attached) + the same fraction of every bin's unattached "
-                      f"clusters ({c.n_unattached}); oracle/tmd_oracle.c orc_decode, single thread, {dt:.2f} s"}
+            "sample": f"{n_s} tracks of the {workload} recipe ({comp.n_attached} attached) + the same fraction of the unattached "
+                      f"clusters ({comp.n_unattached}), encoded by the oracle encoder; oracle/tmd_oracle.c orc_decode, single "
+                      f"thread, {dt:.2f} s"}
 
 
 # ------------------------------------------------------------------------------------------------ clocks
@@ -190,6 +184,25 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ arms
+def aggregate_over_ranks(total_ms: float, n_units: float, device):
+    """Replicas only: every rank decodes its own time frame.  The job's time is the MAX over ranks of the
+    device time, its work the SUM of the units; no collective on the data path.  Works on any backend (NCCL on GPUs,
+    gloo in the CPU test)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return total_ms, n_units
+    t = torch.tensor([total_ms, n_units], dtype=torch.float64, device=device)
+    tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+    return float(tmax[0]), float(tsum[1])
+
+
+def rank_seed_offset(rank: int) -> int:
+    """Rank r decodes time frame r of the recipe (seed + 1000 r): different data, same size class (weak scaling)."""
+    return rank
+
+
 def run_ours(args) -> None:
     import torch
     import torch.distributed as dist
@@ -203,7 +216,7 @@ def run_ours(args) -> None:
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
 
-    geo, arrays = build_workload(args.workload, device, seed_offset=rank)
+    geo, arrays = build_workload(args.workload, device, seed_offset=rank_seed_offset(rank))
     n_trk, n_att, n_un = (int(arrays[k].shape[0]) for k in ("trk_ncl", "a_qtot", "u_qtot"))
     n_cl = n_att + n_un
     ctx = T.tmd_create(geo, BZ)
@@ -236,13 +249,7 @@ def run_ours(args) -> None:
     barrier()
     clocks = sampler.stop() if sampler else None
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
-    t = torch.tensor([total_ms, float(n_cl)], dtype=torch.float64, device=device)
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        total_ms, n_cl_all = float(tmax[0]), float(tsum[1])
-    else:
-        n_cl_all = float(n_cl)
+    total_ms, n_cl_all = aggregate_over_ranks(total_ms, float(n_cl), device)
     ms_per_step = total_ms / args.steps
     value = n_cl_all / (ms_per_step * 1e-3)
     # ---- outside the timed region: the same step with every kernel alone on one stream (TMD_SERIAL), for the
@@ -312,7 +319,7 @@ def run_ours(args) -> None:
             "kernel_gbs_serial": {k: kalg[k] / (kserial[k] * 1e-3) / 1e9 for k in kalg if k in kserial},
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(geo, arrays, n_trk)
+            line["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_tracks, device)
         print(json.dumps(line), flush=True)
     T.tmd_destroy(ctx)
     if world > 1:
@@ -336,33 +343,15 @@ def run_reference(args) -> None:
     if int(os.environ.get("RANK", "0")) != 0:
         return
     import torch
-    from tmd_inputs import build_geometry, physical as ph, timeframe as tf
-    from oracle import tmd_oracle as O
-
-    geo = build_geometry(36)
-    mk, n_un, single = tf.WORKLOADS[args.workload]
-    cfg = mk()
-    n_s = min(cfg.n_tracks, args.ref_tracks)                          # bounded sample: same mix, fewer tracks
-    frac = n_s / cfg.n_tracks
-    cfg.n_tracks = n_s
     dev = "cuda" if torch.cuda.is_available() else "cpu"
-    tr = tf.generate_truth(cfg, geo, dev, batch=200_000)
-    ev_att = tr.att.cpu().numpy().view(ph.CLUSTER_DTYPE).reshape(-1)
-    comp = O.encode(geo, BZ, tr.trk_ncl.cpu().numpy().view(np.uint16), tr.trk_qptf.cpu().numpy(), ev_att, tr.leg.cpu().numpy(),
-                    np.zeros(0, ph.CLUSTER_DTYPE))
-    u = tf.generate_unattached(geo, int(n_un * frac), cfg.seed, dev, "inv_x", single)
-    from tmd_inputs.layout import COMPRESSED_FIELDS, Compressed
-    full = Compressed.empty(comp.n_tracks, comp.n_attached, int(u["u_qtot"].shape[0]), geo.n_bins)
-    for k, (dt, _) in COMPRESSED_FIELDS.items():
-        src = u[k].cpu().numpy().view(np.dtype(dt)) if k in u else getattr(comp, k)
-        getattr(full, k)[:] = src
+    geo, full, n_s = oracle_sample(args.workload, args.ref_tracks, dev)
     n_cl = full.n_attached + full.n_unattached
     for _ in range(args.warmup):
         time_oracle(geo, full)
     dts = [time_oracle(geo, full) for _ in range(args.steps)]
     value = n_cl * len(dts) / sum(dts)
-    sample = (f"{n_s} tracks of the {args.workload} mix ({full.n_attached} attached, {full.n_unattached} unattached) per step; "
-              f"oracle/tmd_oracle.c orc_decode, single thread")
+    sample = (f"{n_s} tracks of the {args.workload} recipe ({full.n_attached} attached, {full.n_unattached} unattached) per step, "
+              f"encoded by the oracle encoder; oracle/tmd_oracle.c orc_decode, single thread")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(dts) / len(dts), "higher_is_better": True,
@@ -382,7 +371,8 @@ def main() -> None:
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4"],
                     help="c3 = full Pb-Pb-scale time frame, the configuration the metric is quoted on")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--ref-tracks", type=int, default=25_000)
+    ap.add_argument("--ref-tracks", type=int, default=25_000, help="tracks per step of the --impl reference arm")
+    ap.add_argument("--cpu-tracks", type=int, default=1_000_000, help="tracks of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -166,7 +166,9 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->rank_smem);
   ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_track_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
+    e = cudaFuncSetAttribute(k_track_decode<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_track_decode<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
   if (e == cudaSuccess) {
     int lo = 0, hi = 0;   // numerically lowest = highest priority: the short integer kernels should not queue behind the decode
@@ -268,7 +270,8 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
     TMD_BEFORE(st);
     const uint32_t decode_blocks = (n_trk + DECODE_THREADS - 1) / DECODE_THREADS;
-    k_track_decode<<<decode_blocks, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
+    if (out->probe_state) k_track_decode<true><<<decode_blocks, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
+    else k_track_decode<false><<<decode_blocks, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
     TMD_AFTER("track_decode", st);
     // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
     RankArgs R;

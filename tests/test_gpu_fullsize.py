@@ -1,0 +1,114 @@
+"""`-m gpu` parity at BASELINE.json's full sizes, in the launch configuration bench.py times (same workload builder, same
+`tmd_decode` call: flags 0, no probes, workspace from `tmd_workspace_bytes`).
+
+A full time frame (c3: 251 M attached + 80 M unattached clusters) is more than the oracle decodes in seconds, so:
+
+1. EVERY output record is compared, on the device with torch library routines only, against what the method's definition
+   fixes at any size -- `decode(encode(x)) == canonical(x)` (pinned for the oracle at small sizes in
+   test_oracle_roundtrip.py): `bin_offset` is the exclusive cumsum of the per-bin counts of the generator's clusters, the
+   attached part of every bin is the generator's clusters in a stable sort by bin, the unattached
+   part is the per-bin cumulative sum of the stored differences (C4).  No expected value comes from the CUDA path.
+2. SAMPLED tracks (random ones, the longest ones, the first and the last) go through the ORACLE one by one: the oracle's
+   encoder, fed with the generator's clusters of the track, must produce the bytes the GPU encoder left in the workload
+   (so the oracle's input is its own), and the oracle's decode of them must equal the records the GPU wrote at the
+   canonical positions of the track's clusters.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+BZ = 0.5
+
+
+def _decode_like_bench(geo, arrays):
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    device = arrays["trk_ncl"].device
+    n_trk, n_att, n_un = (int(arrays[k].shape[0]) for k in ("trk_ncl", "a_qtot", "u_qtot"))
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        clusters = torch.full(((n_att + n_un) * 4,), -0x11111112, dtype=torch.int32, device=device)
+        bin_offset = torch.empty(geo.n_bins + 1, dtype=torch.int32, device=device)
+        ws = torch.empty(T.tmd_workspace_bytes(ctx, n_trk, n_att, n_un), dtype=torch.uint8, device=device)
+        T.tmd_decode(ctx, T.make_compressed(arrays), T.make_output(clusters, bin_offset, ws), 0, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    finally:
+        T.tmd_destroy(ctx)
+    return clusters.view(-1, 4), bin_offset
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4"])
+def test_full_time_frame(name):
+    import torch
+    import bench
+    from oracle import tmd_oracle as O
+    from tmd_inputs import physical as ph, timeframe as tf
+    from tmd_inputs.layout import CLUSTER_DTYPE
+
+    dev = torch.device("cuda", 0)
+    geo, arrays, truth = bench.build_workload(name, dev, keep_truth=True)
+    n_trk, n_att, n_un, n_bins = truth.n_tracks, truth.n_attached, int(arrays["u_qtot"].shape[0]), geo.n_bins
+    got, got_bo = _decode_like_bench(geo, arrays)
+
+    # ---- 1. every record, from the definition (torch library routines on the generator's clusters)
+    w3 = truth.att[:, 3]
+    bins = (((w3 >> 16) & 0xFF) * geo.n_rows + ((w3 >> 8) & 0xFF)).to(torch.int32)
+    att_cnt = torch.bincount(bins, minlength=n_bins)
+    u_cnt = arrays["u_bin_count"].to(torch.int64)
+    want_bo = torch.zeros(n_bins + 1, dtype=torch.int64, device=dev)
+    want_bo[1:] = torch.cumsum(att_cnt + u_cnt, 0)
+    assert torch.equal(got_bo.to(torch.int64) & 0xFFFFFFFF, want_bo), "bin_offset"
+    order = torch.sort(bins, stable=True).indices                     # canonical order of the attached clusters (C5)
+    u_start = torch.cumsum(u_cnt, 0) - u_cnt
+    dest = torch.empty(n_att, dtype=torch.int64, device=dev)           # canonical position of attached cluster g
+    dest[order] = torch.arange(n_att, device=dev) + u_start[bins[order].long()]
+    del order
+    bad = (got[dest] != truth.att).any(dim=1)
+    assert not bool(bad.any()), f"{int(bad.sum())} attached records differ; first g = {int(bad.nonzero()[0])}"
+    del bad
+    # unattached: per-bin running sums of the stored differences (C4), appended after the bin's attached clusters
+    ubin = torch.repeat_interleave(torch.arange(n_bins, device=dev), u_cnt)
+    first = u_start[ubin]
+    i_in = torch.arange(n_un, device=dev) - first
+    cp = torch.cumsum(arrays["u_paddiff"].to(torch.int64) & 0xFFFF, 0)
+    ct = torch.cumsum(arrays["u_timediff"].to(torch.int64) & 0xFFFFFFFF, 0)
+    zero = torch.zeros(1, dtype=torch.int64, device=dev)
+    before_p = torch.cat((zero, cp))[first]
+    before_t = torch.cat((zero, ct))[first]
+    pad = (cp - before_p) & 0xFFFF
+    time = (ct - before_t) & 0xFFFFFFFF
+    del cp, ct, before_p, before_t
+    want_u = tf.pack_records(time, pad, arrays["u_qtot"].to(torch.int64) & 0xFFFF, arrays["u_qmax"].to(torch.int64) & 0xFFFF,
+                             arrays["u_sigpad"].to(torch.int64), arrays["u_sigtime"].to(torch.int64),
+                             arrays["u_flags"].to(torch.int64), ubin % geo.n_rows, ubin // geo.n_rows)
+    udest = want_bo[ubin] + att_cnt[ubin] + i_in
+    bad = (got[udest] != want_u).any(dim=1)
+    assert not bool(bad.any()), f"{int(bad.sum())} unattached records differ"
+    del bad, want_u, udest, ubin, first, i_in, pad, time
+
+    # ---- 2. sampled tracks through the oracle, one by one
+    rng = np.random.default_rng(7)
+    ncl = (truth.trk_ncl.to(torch.int64) & 0xFFFF)
+    off = torch.cumsum(ncl, 0) - ncl
+    longest = torch.topk(ncl, 16).indices.cpu().numpy()
+    sample = np.unique(np.concatenate((rng.integers(0, n_trk, 400), longest, [0, n_trk - 1])))
+    h_off, h_ncl = off.cpu().numpy(), ncl.cpu().numpy()
+    res_fields = ("a_rowdiff", "a_secleg", "a_padres", "a_timeres")
+    for t in sample:
+        g0, n = int(h_off[t]), int(h_ncl[t])
+        att = truth.att[g0:g0 + n].cpu().numpy().view(CLUSTER_DTYPE).reshape(-1)
+        leg = truth.leg[g0:g0 + n].cpu().numpy()
+        comp = O.encode(geo, BZ, np.array([n], np.uint16), truth.trk_qptf[t:t + 1].cpu().numpy(), att, leg, np.zeros(0, CLUSTER_DTYPE))
+        r0 = g0 - int(t)
+        for k in res_fields:                                            # the GPU-encoded streams are the oracle's own bytes
+            mine = arrays[k][r0:r0 + n - 1].cpu().numpy().view(getattr(comp, k).dtype)
+            assert np.array_equal(mine, getattr(comp, k)), f"track {t}: {k}"
+        for k in ("trk_qpt", "trk_row0", "trk_sec0", "trk_pad0", "trk_time0"):
+            assert arrays[k][t:t + 1].cpu().numpy().view(getattr(comp, k).dtype)[0] == getattr(comp, k)[0], f"track {t}: {k}"
+        d = O.decode_track(geo, BZ, int(comp.trk_qpt[0]), int(comp.trk_sec0[0]), int(comp.trk_row0[0]), int(comp.trk_pad0[0]),
+                           int(comp.trk_time0[0]), comp.a_rowdiff, comp.a_secleg, comp.a_padres, comp.a_timeres)
+        rec = got[dest[g0:g0 + n]].cpu().numpy().view(CLUSTER_DTYPE).reshape(-1)
+        for f, key in (("sector", "sec"), ("row", "row"), ("pad", "P"), ("time", "T")):
+            assert np.array_equal(rec[f], d[key]), f"track {t}: {f}"
+        for f in ("qtot", "qmax", "sigpad", "sigtime", "flags"):
+            assert np.array_equal(rec[f], att[f]), f"track {t}: {f}"

@@ -181,16 +181,22 @@ def test_gpu_encoder_matches_oracle_encoder(phys_case):
 
 
 def test_bench_workload_builder_matches_oracle():
-    # the path bench.py times: torch helix truth -> GPU encoder -> GPU decoder, against the oracle on the same arrays
+    # the path bench.py times: torch helix truth -> GPU encoder -> GPU decoder.  The oracle gets the generator's clusters
+    # and its OWN encoder's bytes; the GPU encoder's bytes must be the same, then both decoders must agree.
     import torch
     import bench
-    from tmd_inputs import timeframe as tf
-    from tmd_inputs.layout import COMPRESSED_FIELDS
-    saved = tf.WORKLOADS["c1"]
-    geo, arrays = bench.build_workload("c1", torch.device("cuda", 0))
-    comp = Compressed.empty(int(arrays["trk_ncl"].shape[0]), int(arrays["a_qtot"].shape[0]), int(arrays["u_qtot"].shape[0]), geo.n_bins)
-    for k, (dt, _) in COMPRESSED_FIELDS.items():
-        getattr(comp, k)[:] = arrays[k].cpu().numpy().view(np.dtype(dt))
+    from tmd_inputs.layout import CLUSTER_DTYPE, COMPRESSED_FIELDS
+    geo, arrays, truth = bench.build_workload("c1", torch.device("cuda", 0), keep_truth=True)
+    att = truth.att.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1)
+    comp = O.encode(geo, BZ, truth.trk_ncl.cpu().numpy().view(np.uint16), truth.trk_qptf.cpu().numpy(), att, truth.leg.cpu().numpy(),
+                    np.zeros(0, CLUSTER_DTYPE))
     assert comp.n_tracks == 10_000 and 1.1e6 < comp.n_attached < 1.4e6
-    assert_same(gpu_decode(geo, BZ, comp, probe_step=0xFFFFFFFF), O.decode(geo, BZ, comp, probe_step=0xFFFFFFFF))
-    assert tf.WORKLOADS["c1"] is saved
+    full = Compressed.empty(comp.n_tracks, comp.n_attached, int(arrays["u_qtot"].shape[0]), geo.n_bins)
+    for k, (dt, which) in COMPRESSED_FIELDS.items():
+        mine = arrays[k].cpu().numpy().view(np.dtype(dt))
+        if which in ("n_tracks", "n_attached", "n_residuals"):
+            assert np.array_equal(mine, getattr(comp, k)), f"GPU encoder, {k}: " + first_mismatch(mine, getattr(comp, k))
+            getattr(full, k)[:] = getattr(comp, k)
+        else:
+            getattr(full, k)[:] = mine                    # unattached: drawn in the compressed domain by the generator
+    assert_same(gpu_decode(geo, BZ, full, probe_step=0xFFFFFFFF), O.decode(geo, BZ, full, probe_step=0xFFFFFFFF))
