@@ -42,20 +42,18 @@ struct WalkState {
   int dir;
 };
 
-__device__ __forceinline__ uint32_t reduce_mod(uint32_t v, uint32_t m) {  // v < 256, m >= 1 (reading 19)
-  while (v >= m) v -= m;
-  return v;
-}
+// v mod m by multiplication (reading 19): magic = floor(2^24 / m) + 1 is exact for v * m < 2^24 (v < 256 here)
+__device__ __forceinline__ uint32_t reduce_mod(uint32_t v, uint32_t m, uint32_t magic) { return v - ((v * magic) >> 24) * m; }
 
 // returns the reduced sector step d (0 = same sector); updates row / az / dir
-__device__ __forceinline__ uint32_t walk_step(WalkState& w, uint32_t rowdiff, uint32_t secleg, uint32_t n_rows, uint32_t n_az) {
+__device__ __forceinline__ uint32_t walk_step(WalkState& w, uint32_t rowdiff, uint32_t secleg, const DevGeo& G) {
   if (secleg & 0x80u) w.dir = -w.dir;
-  uint32_t rd = reduce_mod(rowdiff, n_rows);
-  uint32_t r = w.row + (w.dir > 0 ? rd : n_rows - rd);
-  w.row = r >= n_rows ? r - n_rows : r;
-  uint32_t d = reduce_mod(secleg & 0x3Fu, n_az);
-  uint32_t a = w.az + d;
-  w.az = a >= n_az ? a - n_az : a;
+  const uint32_t rd = reduce_mod(rowdiff, G.n_rows, G.rows_magic);
+  const uint32_t r = w.row + (w.dir > 0 ? rd : G.n_rows - rd);
+  w.row = r >= G.n_rows ? r - G.n_rows : r;
+  const uint32_t d = reduce_mod(secleg & 0x3Fu, G.n_az, G.az_magic);
+  const uint32_t a = w.az + d;
+  w.az = a >= G.n_az ? a - G.n_az : a;
   return d;
 }
 
