@@ -298,6 +298,12 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   TMD_BEFORE(st);
   k_bin_offsets<<<1, 1024, 0, st>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
   TMD_AFTER("bin_offsets", st);
+  if (n_trk > 0) {
+    dim3 cg((n_bins + 255) / 256, W.n_groups);
+    TMD_BEFORE(st);
+    k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
+    TMD_AFTER("col_apply", st);
+  }
   // ---- fork: A7 (unattached clusters) on the context's second stream, next to A6 on the caller's
   const bool fork = n_un > 0 && n_trk > 0 && s2 != st;
   if (n_un > 0) {
@@ -315,10 +321,6 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     if (fork) TMD_CUDA(cudaEventRecord(ctx->ev_join, s2));
   }
   if (n_trk > 0) {
-    dim3 cg((n_bins + 255) / 256, W.n_groups);
-    TMD_BEFORE(st);
-    k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
-    TMD_AFTER("col_apply", st);
     // A6: copy-through + scatter
     ScatterArgs S;
     S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
