@@ -10,8 +10,8 @@
 // no atomics, no sort, and the result is the sequential one by construction.  The 32 clusters are cut into runs of
 // strictly ascending (or descending) bins, inside which all bins differ, so one conflict-free load / store round serves
 // a run; consecutive clusters of a track lie on consecutive pad rows, so a round handles ~32 clusters (adversarial
-// inputs degrade to one cluster per round, still exact).  The records of the next 8 groups are loaded while the
-// current 8 are ranked.
+// inputs degrade to one cluster per round, still exact).  The records of the next 16 groups are loaded while the
+// current 16 are ranked.
 #pragma once
 
 #include "tmd_common.cuh"
@@ -20,7 +20,7 @@ namespace tmd {
 
 constexpr int WR_WARPS = 4;                            // warps per block (each with its own chunk and counters)
 constexpr int WR_THREADS = WR_WARPS * 32;
-constexpr int WR_DEPTH = 8;                            // groups of 32 clusters loaded ahead
+constexpr int WR_DEPTH = 16;                           // groups of 32 clusters loaded ahead
 
 struct RankArgs {
   const uint2* inter;           // [n_attached] intermediate records of the track-decode kernel; bin = .y >> 16

@@ -23,41 +23,68 @@ struct UnattachedArgs {
 constexpr int UNATT_THREADS = 256;
 constexpr int UNATT_ITEMS = 4;
 
-// v1: one block per bin, tiles of UNATT_THREADS * UNATT_ITEMS consecutive clusters, block scan with a running carry.
+// One block per bin; tiles of UNATT_THREADS * 4 consecutive clusters, aligned to 4 in the global cluster index so that
+// every stream is read with one vector load per thread (8 B of pad differences, 16 B of time differences, 8 + 8 B of
+// charges, 3 x 4 B of widths / flags); block scan of the per-thread sums with a running carry; 4 x 16-byte stores per thread.
 __global__ void __launch_bounds__(UNATT_THREADS) k_unattached(DevGeo G, UnattachedArgs A) {
   __shared__ uint32_t ws[33];
   const uint32_t b = blockIdx.x;
-  const uint32_t i0 = A.u_start[b], cnt = A.u_start[b + 1] - i0;
-  if (cnt == 0) return;
+  const uint32_t i0 = A.u_start[b], i1 = A.u_start[b + 1];
+  if (i1 == i0) return;
+  const uint32_t n_un = (uint32_t)A.in.n_unattached;
   const uint32_t dst0 = A.bin_offset[b] + A.att_cnt[b];
   const uint32_t sec = b / G.n_rows, row = b - sec * G.n_rows;
+  const uint32_t tail = (row << 8) | (sec << 16);
   uint32_t carry_p = 0, carry_t = 0;
-  for (uint32_t base = 0; base < cnt; base += UNATT_THREADS * UNATT_ITEMS) {
-    const uint32_t k0 = base + threadIdx.x * UNATT_ITEMS;
-    uint32_t p[UNATT_ITEMS], t[UNATT_ITEMS];
-    uint32_t sp = 0, st = 0;
+  for (uint32_t base = i0 & ~3u; base < i1; base += UNATT_THREADS * UNATT_ITEMS) {
+    const uint32_t k0 = base + threadIdx.x * UNATT_ITEMS;        // multiple of 4
+    uint32_t pd[4] = {0, 0, 0, 0}, td[4] = {0, 0, 0, 0}, qt[4], qm[4], sp[4], st[4], fl[4];
+    if (k0 < i1 && k0 + 4 > i0) {
+      if (k0 + 4 <= n_un) {
+        const uint2 p2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_paddiff + k0));
+        const uint4 t4 = __ldg(reinterpret_cast<const uint4*>(A.in.u_timediff + k0));
+        const uint2 q2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_qtot + k0));
+        const uint2 m2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_qmax + k0));
+        const uint32_t a = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_sigpad + k0));
+        const uint32_t c = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_sigtime + k0));
+        const uint32_t f = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_flags + k0));
+        pd[0] = p2.x & 0xFFFFu; pd[1] = p2.x >> 16; pd[2] = p2.y & 0xFFFFu; pd[3] = p2.y >> 16;
+        td[0] = t4.x; td[1] = t4.y; td[2] = t4.z; td[3] = t4.w;
+        qt[0] = q2.x & 0xFFFFu; qt[1] = q2.x >> 16; qt[2] = q2.y & 0xFFFFu; qt[3] = q2.y >> 16;
+        qm[0] = m2.x & 0xFFFFu; qm[1] = m2.x >> 16; qm[2] = m2.y & 0xFFFFu; qm[3] = m2.y >> 16;
 #pragma unroll
-    for (int k = 0; k < UNATT_ITEMS; ++k) {
-      const bool in = k0 + k < cnt;
-      sp += in ? A.in.u_paddiff[i0 + k0 + k] : 0u;
-      st += in ? A.in.u_timediff[i0 + k0 + k] : 0u;
-      p[k] = sp;
-      t[k] = st;
+        for (int k = 0; k < 4; ++k) { sp[k] = (a >> (8 * k)) & 0xFFu; st[k] = (c >> (8 * k)) & 0xFFu; fl[k] = (f >> (8 * k)) & 0xFFu; }
+      } else {                                                   // the last clusters of the arrays
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const uint32_t i = min(k0 + k, n_un - 1);
+          pd[k] = A.in.u_paddiff[i]; td[k] = A.in.u_timediff[i]; qt[k] = A.in.u_qtot[i]; qm[k] = A.in.u_qmax[i];
+          sp[k] = A.in.u_sigpad[i]; st[k] = A.in.u_sigtime[i]; fl[k] = A.in.u_flags[i];
+        }
+      }
+    }
+    uint32_t sum_p = 0, sum_t = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const bool in = k0 + k >= i0 && k0 + k < i1;               // clusters of neighbouring bins in the vector do not count
+      sum_p += in ? pd[k] : 0u;
+      sum_t += in ? td[k] : 0u;
+      pd[k] = sum_p;
+      td[k] = sum_t;
     }
     uint32_t tot_p, tot_t;
-    const uint32_t ex_p = carry_p + block_excl_scan(sp, ws, &tot_p);
-    const uint32_t ex_t = carry_t + block_excl_scan(st, ws, &tot_t);
+    const uint32_t ex_p = carry_p + block_excl_scan(sum_p, ws, &tot_p);
+    const uint32_t ex_t = carry_t + block_excl_scan(sum_t, ws, &tot_t);
 #pragma unroll
-    for (int k = 0; k < UNATT_ITEMS; ++k) {
+    for (int k = 0; k < 4; ++k) {
       const uint32_t i = k0 + k;
-      if (i < cnt && dst0 + i < A.n_clusters_total) {
-        const size_t s = (size_t)i0 + i;
+      if (i >= i0 && i < i1 && dst0 + (i - i0) < A.n_clusters_total) {
         uint4 v;
-        v.x = ex_t + t[k];
-        v.y = ((ex_p + p[k]) & 0xFFFFu) | ((uint32_t)A.in.u_qtot[s] << 16);
-        v.z = (uint32_t)A.in.u_qmax[s] | ((uint32_t)A.in.u_sigpad[s] << 16) | ((uint32_t)A.in.u_sigtime[s] << 24);
-        v.w = (uint32_t)A.in.u_flags[s] | (row << 8) | (sec << 16);
-        A.clusters[dst0 + i] = v;
+        v.x = ex_t + td[k];
+        v.y = ((ex_p + pd[k]) & 0xFFFFu) | (qt[k] << 16);
+        v.z = qm[k] | (sp[k] << 16) | (st[k] << 24);
+        v.w = fl[k] | tail;
+        A.clusters[dst0 + (i - i0)] = v;
       }
     }
     carry_p += tot_p;
