@@ -162,6 +162,20 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
  */
 int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream);
 
+/*
+ * Pipelined form of tmd_decode_host (the deployment shape of PAPER.md L64 / L70: "multiple instances are executed
+ * concurrently on different streams, reducing the memory transfer latency").  The context owns TMD_HOST_SLOTS device
+ * arenas and three streams (uploads, decode, downloads).  tmd_decode_host_async enqueues the upload, the decode and the
+ * download of one time frame in slot `slot` (0 .. TMD_HOST_SLOTS-1) and returns; if the slot still holds an earlier
+ * frame it first waits for that frame's download.  With two slots used alternately the upload of frame i+1 runs beside
+ * the download of frame i.  HOST pointers as in tmd_decode_host; they must be pinned for the copies to overlap and must
+ * stay valid until tmd_host_wait(slot) returns.  TMD_VALIDATE is not accepted (it synchronises): TMD_ERR_ARG.
+ * tmd_host_wait blocks until the frame in `slot` is complete in the host buffers (no-op for an idle slot).
+ */
+#define TMD_HOST_SLOTS 2
+int tmd_decode_host_async(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot);
+int tmd_host_wait(tmd_ctx* ctx, int slot);
+
 /* Frees the context and its device tables / buffers.  Null is accepted. */
 int tmd_destroy(tmd_ctx* ctx);
 

@@ -28,9 +28,17 @@ struct tmd_ctx {
   cudaEvent_t ev_t0[TMD_MAX_KERNELS], ev_t1[TMD_MAX_KERNELS];
   const char* kernel_names[TMD_MAX_KERNELS];
   bool events_created, timing_valid;
-  // arena of tmd_decode_host (grown on demand)
-  void* arena;
-  size_t arena_bytes;
+  // tmd_decode_host / tmd_decode_host_async: TMD_HOST_SLOTS frames in flight, each with its own device arena (inputs,
+  // outputs, workspace; grown on demand); host->device copies, decode and device->host copies on three streams so that
+  // the upload of one frame overlaps the download of the previous one (Fig. 2: transfers beside kernels)
+  struct HostSlot {
+    void* arena;
+    size_t arena_bytes;
+    cudaEvent_t h2d_done, dec_done, d2h_done;
+    bool busy;
+  } slots[TMD_HOST_SLOTS];
+  cudaStream_t s_h2d, s_dec, s_d2h;
+  bool host_ready;
   size_t decode_smem, rank_smem;
   int n_sm;
 };
@@ -396,9 +404,18 @@ int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compress
   return TMD_OK;
 }
 
-int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
+// Enqueue one host-to-host decode in slot `slot`: copies in on `s_in`, decode on `s_run`, copies out on `s_out` (the three
+// may be the same stream), ordered by the slot's events.  Does not wait for the result.
+static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot, cudaStream_t s_in,
+                        cudaStream_t s_run, cudaStream_t s_out) {
   int rc = check_args(ctx, in, out, false);
   if (rc != TMD_OK) return rc;
+  tmd_ctx::HostSlot& S = ctx->slots[slot];
+  if (!S.h2d_done) {
+    TMD_CUDA(cudaEventCreateWithFlags(&S.h2d_done, cudaEventDisableTiming));
+    TMD_CUDA(cudaEventCreateWithFlags(&S.dec_done, cudaEventDisableTiming));
+    TMD_CUDA(cudaEventCreateWithFlags(&S.d2h_done, cudaEventDisableTiming));
+  }
   const uint32_t n_bins = ctx->geo.n_bins;
   const size_t n_trk = in->n_tracks, n_att = in->n_attached, n_res = n_att - n_trk, n_un = in->n_unattached;
   const Workspace W = layout(n_bins, in->n_tracks, n_att);
@@ -407,9 +424,9 @@ int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uin
   Seg segs[] = {
       {in->trk_ncl, n_trk * 2, 0},   {in->trk_qpt, n_trk, 0},      {in->trk_row0, n_trk, 0},    {in->trk_sec0, n_trk, 0},
       {in->trk_pad0, n_trk * 2, 0},  {in->trk_time0, n_trk * 4, 0},
+      {in->a_rowdiff, n_res, 0},     {in->a_secleg, n_res, 0},     {in->a_padres, n_res * 2, 0}, {in->a_timeres, n_res * 4, 0},
       {in->a_qtot, n_att * 2, 0},    {in->a_qmax, n_att * 2, 0},   {in->a_flags, n_att, 0},     {in->a_sigpad, n_att, 0},
       {in->a_sigtime, n_att, 0},
-      {in->a_rowdiff, n_res, 0},     {in->a_secleg, n_res, 0},     {in->a_padres, n_res * 2, 0}, {in->a_timeres, n_res * 4, 0},
       {in->u_qtot, n_un * 2, 0},     {in->u_qmax, n_un * 2, 0},    {in->u_flags, n_un, 0},      {in->u_sigpad, n_un, 0},
       {in->u_sigtime, n_un, 0},      {in->u_paddiff, n_un * 2, 0}, {in->u_timediff, n_un * 4, 0},
       {in->u_bin_count, (size_t)n_bins * 4, 0}};
@@ -419,21 +436,24 @@ int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uin
   const size_t o_binoff = o;   o += align_up(((size_t)n_bins + 1) * 4);
   const size_t o_probe = o;    o += align_up(out->probe_state ? n_trk * 24 : 0);
   const size_t o_ws = o;       o += W.total;
-  if (o > ctx->arena_bytes) {
-    if (ctx->arena) cudaFree(ctx->arena);
-    ctx->arena = nullptr; ctx->arena_bytes = 0;
-    if (cudaMalloc(&ctx->arena, o) != cudaSuccess) { cudaGetLastError(); return TMD_ERR_CUDA; }
-    ctx->arena_bytes = o;
+  if (S.busy) {                                   // the slot's previous frame must have left the arena
+    TMD_CUDA(cudaEventSynchronize(S.d2h_done));
+    S.busy = false;
   }
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  unsigned char* a = (unsigned char*)ctx->arena;
+  if (o > S.arena_bytes) {
+    if (S.arena) cudaFree(S.arena);
+    S.arena = nullptr; S.arena_bytes = 0;
+    if (cudaMalloc(&S.arena, o) != cudaSuccess) { cudaGetLastError(); return TMD_ERR_CUDA; }
+    S.arena_bytes = o;
+  }
+  unsigned char* a = (unsigned char*)S.arena;
   for (const Seg& s : segs)
-    if (s.bytes && cudaMemcpyAsync(a + s.at, s.src, s.bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TMD_ERR_CUDA;
+    if (s.bytes) TMD_CUDA(cudaMemcpyAsync(a + s.at, s.src, s.bytes, cudaMemcpyHostToDevice, s_in));
   tmd_compressed d = *in;
   const void** dst[] = {(const void**)&d.trk_ncl, (const void**)&d.trk_qpt, (const void**)&d.trk_row0, (const void**)&d.trk_sec0,
-                        (const void**)&d.trk_pad0, (const void**)&d.trk_time0, (const void**)&d.a_qtot, (const void**)&d.a_qmax,
-                        (const void**)&d.a_flags, (const void**)&d.a_sigpad, (const void**)&d.a_sigtime, (const void**)&d.a_rowdiff,
-                        (const void**)&d.a_secleg, (const void**)&d.a_padres, (const void**)&d.a_timeres, (const void**)&d.u_qtot,
+                        (const void**)&d.trk_pad0, (const void**)&d.trk_time0, (const void**)&d.a_rowdiff, (const void**)&d.a_secleg,
+                        (const void**)&d.a_padres, (const void**)&d.a_timeres, (const void**)&d.a_qtot, (const void**)&d.a_qmax,
+                        (const void**)&d.a_flags, (const void**)&d.a_sigpad, (const void**)&d.a_sigtime, (const void**)&d.u_qtot,
                         (const void**)&d.u_qmax, (const void**)&d.u_flags, (const void**)&d.u_sigpad, (const void**)&d.u_sigtime,
                         (const void**)&d.u_paddiff, (const void**)&d.u_timediff, (const void**)&d.u_bin_count};
   for (size_t i = 0; i < sizeof(segs) / sizeof(segs[0]); ++i) *dst[i] = a + segs[i].at;
@@ -443,16 +463,50 @@ int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uin
   dout.probe_state = out->probe_state ? (uint32_t*)(a + o_probe) : nullptr;
   dout.workspace = a + o_ws;
   dout.workspace_bytes = W.total;
-  rc = tmd_decode(ctx, &d, &dout, flags, cuda_stream);
+  if (s_run != s_in) {
+    TMD_CUDA(cudaEventRecord(S.h2d_done, s_in));
+    TMD_CUDA(cudaStreamWaitEvent(s_run, S.h2d_done, 0));
+  }
+  rc = tmd_decode(ctx, &d, &dout, flags, (void*)s_run);
   if (rc != TMD_OK) return rc;
-  if ((n_att + n_un) && cudaMemcpyAsync(out->clusters, dout.clusters, (n_att + n_un) * 16, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-    return TMD_ERR_CUDA;
-  if (cudaMemcpyAsync(out->bin_offset, dout.bin_offset, ((size_t)n_bins + 1) * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-    return TMD_ERR_CUDA;
-  if (out->probe_state && n_trk &&
-      cudaMemcpyAsync(out->probe_state, dout.probe_state, n_trk * 24, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-    return TMD_ERR_CUDA;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
+  if (s_out != s_run) {
+    TMD_CUDA(cudaEventRecord(S.dec_done, s_run));
+    TMD_CUDA(cudaStreamWaitEvent(s_out, S.dec_done, 0));
+  }
+  if (n_att + n_un) TMD_CUDA(cudaMemcpyAsync(out->clusters, dout.clusters, (n_att + n_un) * 16, cudaMemcpyDeviceToHost, s_out));
+  TMD_CUDA(cudaMemcpyAsync(out->bin_offset, dout.bin_offset, ((size_t)n_bins + 1) * 4, cudaMemcpyDeviceToHost, s_out));
+  if (out->probe_state && n_trk)
+    TMD_CUDA(cudaMemcpyAsync(out->probe_state, dout.probe_state, n_trk * 24, cudaMemcpyDeviceToHost, s_out));
+  TMD_CUDA(cudaEventRecord(S.d2h_done, s_out));
+  S.busy = true;
+  return TMD_OK;
+}
+
+int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
+  if (!ctx) return TMD_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = host_enqueue(ctx, in, out, flags, 0, st, st, st);
+  if (rc != TMD_OK) return rc;
+  return tmd_host_wait(ctx, 0);
+}
+
+int tmd_decode_host_async(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot) {
+  if (!ctx || slot < 0 || slot >= TMD_HOST_SLOTS || (flags & TMD_VALIDATE)) return TMD_ERR_ARG;
+  if (!ctx->host_ready) {
+    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
+    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_dec, cudaStreamNonBlocking));
+    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+    ctx->host_ready = true;
+  }
+  return host_enqueue(ctx, in, out, flags, slot, ctx->s_h2d, ctx->s_dec, ctx->s_d2h);
+}
+
+int tmd_host_wait(tmd_ctx* ctx, int slot) {
+  if (!ctx || slot < 0 || slot >= TMD_HOST_SLOTS) return TMD_ERR_ARG;
+  tmd_ctx::HostSlot& S = ctx->slots[slot];
+  if (!S.busy) return TMD_OK;
+  TMD_CUDA(cudaEventSynchronize(S.d2h_done));
+  S.busy = false;
   return TMD_OK;
 }
 
@@ -461,7 +515,12 @@ int tmd_destroy(tmd_ctx* ctx) {
   if (ctx->side) { cudaStreamSynchronize(ctx->side); cudaStreamDestroy(ctx->side); }
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
-  if (ctx->arena) cudaFree(ctx->arena);
+  for (tmd_ctx::HostSlot& S : ctx->slots) {
+    if (S.busy) cudaEventSynchronize(S.d2h_done);
+    if (S.arena) cudaFree(S.arena);
+    if (S.h2d_done) { cudaEventDestroy(S.h2d_done); cudaEventDestroy(S.dec_done); cudaEventDestroy(S.d2h_done); }
+  }
+  if (ctx->host_ready) { cudaStreamDestroy(ctx->s_h2d); cudaStreamDestroy(ctx->s_dec); cudaStreamDestroy(ctx->s_d2h); }
   if (ctx->d_rows) cudaFree(ctx->d_rows);
   if (ctx->events_created)
     for (int i = 0; i < TMD_MAX_KERNELS; ++i) { cudaEventDestroy(ctx->ev_t0[i]); cudaEventDestroy(ctx->ev_t1[i]); }

@@ -20,6 +20,7 @@ TMD_VALIDATE = 1
 TMD_TIMING = 2
 TMD_SERIAL = 4
 TMD_MAX_KERNELS = 24
+TMD_HOST_SLOTS = 2
 PROBE_FINAL = 0xFFFFFFFF
 
 # (field name, numpy dtype) in the order of struct tmd_compressed
@@ -77,6 +78,10 @@ def lib() -> C.CDLL:
         L.tmd_kernel_times.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
         L.tmd_encode_attached.argtypes = [C.c_void_p, C.POINTER(tmd_attached_truth), C.POINTER(tmd_compressed), C.c_void_p,
                                           C.c_size_t, C.c_void_p]
+        L.tmd_decode_host_async.argtypes = [C.c_void_p, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_int]
+        L.tmd_host_wait.argtypes = [C.c_void_p, C.c_int]
+        L.tmd_decode_host_async.restype = C.c_int
+        L.tmd_host_wait.restype = C.c_int
         L.tmd_kernel_times.restype = C.c_int
         L.tmd_encode_attached.restype = C.c_int
         for f in (L.tmd_create, L.tmd_workspace_bytes, L.tmd_decode, L.tmd_decode_host, L.tmd_destroy, L.tmd_last_launch_count):
@@ -161,6 +166,16 @@ def tmd_decode(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, 
 def tmd_decode_host(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, stream: int = 0) -> None:
     """End-to-end decode with HOST pointers (copies in, decodes, copies out, synchronises)."""
     _check(lib().tmd_decode_host(ctx, C.byref(comp), C.byref(out), flags, stream))
+
+
+def tmd_decode_host_async(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, slot: int = 0) -> None:
+    """Enqueue upload + decode + download of one time frame (pinned HOST pointers) in pipeline slot `slot`; returns at once."""
+    _check(lib().tmd_decode_host_async(ctx, C.byref(comp), C.byref(out), flags, slot))
+
+
+def tmd_host_wait(ctx: int, slot: int = 0) -> None:
+    """Block until the frame in pipeline slot `slot` is complete in its host buffers."""
+    _check(lib().tmd_host_wait(ctx, slot))
 
 
 def tmd_kernel_times(ctx: int) -> list[tuple[str, float]]:

@@ -200,3 +200,34 @@ def test_bench_workload_builder_matches_oracle():
         else:
             getattr(full, k)[:] = mine                    # unattached: drawn in the compressed domain by the generator
     assert_same(gpu_decode(geo, BZ, full, probe_step=0xFFFFFFFF), O.decode(geo, BZ, full, probe_step=0xFFFFFFFF))
+
+
+def test_pipelined_host_entry_points_match():
+    # tmd_decode_host_async / tmd_host_wait: frames alternate between the two slots; each result equals the oracle's
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs.layout import CLUSTER_DTYPE, COMPRESSED_FIELDS
+    from gpu_util import _as_torch
+    geo = build_geometry(36)
+    frames = [random_compressed(geo, 3000, 20_000, 41, max_ncl=200), random_compressed(geo, 500, 90_000, 42, max_ncl=60),
+              random_compressed(geo, 4000, 1000, 43, max_ncl=150)]
+    want = [O.decode(geo, BZ, c) for c in frames]
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        held = []
+        for i, c in enumerate(frames):
+            h_in = {k: _as_torch(np.ascontiguousarray(getattr(c, k))).pin_memory() for k in COMPRESSED_FIELDS}
+            n = c.n_attached + c.n_unattached
+            hc = torch.zeros(n * 16, dtype=torch.uint8).pin_memory()
+            hb = torch.zeros(geo.n_bins + 1, dtype=torch.int32).pin_memory()
+            held.append((h_in, hc, hb))
+            T.tmd_decode_host_async(ctx, T.make_compressed(h_in), T.make_output(hc, hb), 0, i % T.TMD_HOST_SLOTS)
+        for s_ in range(T.TMD_HOST_SLOTS):
+            T.tmd_host_wait(ctx, s_)
+        for (h_in, hc, hb), (w_cl, w_bo, _) in zip(held, want):
+            assert np.array_equal(hb.numpy().view(np.uint32), w_bo)
+            assert hc.numpy().view(CLUSTER_DTYPE).tobytes() == w_cl.tobytes()
+        with pytest.raises(T.TmdError):
+            T.tmd_decode_host_async(ctx, T.make_compressed(held[0][0]), T.make_output(held[0][1], held[0][2]), T.TMD_VALIDATE, 0)
+    finally:
+        T.tmd_destroy(ctx)
