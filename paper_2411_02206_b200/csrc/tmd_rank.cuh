@@ -35,12 +35,25 @@ __host__ __device__ inline uint32_t wr_warp_smem(uint32_t n_bins) { return (n_bi
 // Rank of 32 consecutive clusters (lane order) with bins b (BIN_INVALID = no output bin) against the warp's counters:
 // rank = cnt[b]++ executed in lane order.  The 32 clusters are cut into runs of strictly ascending bins (or strictly
 // descending ones, whichever gives fewer runs); inside a run all bins differ, so one load / store round serves it.
-__device__ __forceinline__ uint32_t warp_rank32(uint16_t* cnt, uint32_t b, uint32_t lane) {
+// warp_runs computes the run starts (no shared memory: independent between groups, so a batch of groups is done at once);
+// warp_rank32 does the rounds, which are the only sequential part.
+__device__ __forceinline__ uint32_t warp_runs(uint32_t b, uint32_t lane) {
   const uint32_t prev = __shfl_up_sync(0xffffffffu, b, 1);
   const uint32_t brk_a = __ballot_sync(0xffffffffu, lane == 0 || !(b > prev));
   const uint32_t brk_d = __ballot_sync(0xffffffffu, lane == 0 || !(b < prev));
-  uint32_t brk = __popc(brk_a) <= __popc(brk_d) ? brk_a : brk_d;   // bit l: lane l starts a run (bit 0 always set)
+  return __popc(brk_a) <= __popc(brk_d) ? brk_a : brk_d;          // bit l: lane l starts a run (bit 0 always set)
+}
+
+__device__ __forceinline__ uint32_t warp_rank32(uint16_t* cnt, uint32_t b, uint32_t brk, uint32_t lane) {
   uint32_t rank = 0;
+  if (brk == 1u) {                                                 // one run: the usual case
+    if (b != BIN_INVALID) {
+      rank = cnt[b];
+      cnt[b] = (uint16_t)(rank + 1);
+    }
+    __syncwarp();
+    return rank;
+  }
   while (brk) {
     const uint32_t lo = __ffs(brk) - 1;
     brk &= brk - 1;
@@ -70,19 +83,22 @@ __global__ void __launch_bounds__(WR_THREADS) k_rank(DevGeo G, RankArgs A) {
 #pragma unroll
     for (int k = 0; k < WR_DEPTH; ++k) {
       const uint32_t g = g0 + k * 32 + lane;
-      cur[k] = g < g1 ? __ldg(&A.inter[g].y) >> 16 : (uint32_t)BIN_INVALID;
+      cur[k] = g < g1 ? __ldg(&A.inter[g].y) : 0xFFFFFFFFu;         // raw word: the bin is taken at the use, not here
     }
     for (uint32_t gb = g0; gb < g1; gb += WR_DEPTH * 32) {
 #pragma unroll
       for (int k = 0; k < WR_DEPTH; ++k) {
         const uint32_t g = gb + (WR_DEPTH + k) * 32 + lane;
-        nxt[k] = g < g1 ? __ldg(&A.inter[g].y) >> 16 : (uint32_t)BIN_INVALID;
+        nxt[k] = g < g1 ? __ldg(&A.inter[g].y) : 0xFFFFFFFFu;       // no use of the value before the next batch
       }
+      uint32_t runs[WR_DEPTH];
+#pragma unroll
+      for (int k = 0; k < WR_DEPTH; ++k) runs[k] = warp_runs(cur[k] >> 16, lane);
 #pragma unroll
       for (int k = 0; k < WR_DEPTH; ++k) {
         const uint32_t g = gb + k * 32 + lane;
         if (gb + k * 32 < g1) {                                   // warp-uniform
-          const uint32_t rank = warp_rank32(cnt, cur[k], lane);
+          const uint32_t rank = warp_rank32(cnt, cur[k] >> 16, runs[k], lane);
           if (g < g1) A.rank16[g] = (uint16_t)rank;
         }
       }
