@@ -315,7 +315,7 @@ def run_ours(args) -> None:
                     "algorithmic_bytes_per_launch": alg, "kernel_ms": kserial[dom],
                     "kernel_ms_in_timed_region": kavg.get(dom),
                     "note": "kernel timed alone on one stream (TMD_SERIAL pass after the timed region); in the timed region "
-                            "it overlaps the integer kernels of the second stream"}
+                            "it shares the GPU with the unattached kernel of the second stream"}
         total_alg = algorithmic_bytes_attached(n_trk, n_att) + algorithmic_bytes_unattached(n_un, geo.n_bins)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -36,7 +36,9 @@ typedef enum {
   TMD_ERR_CORRUPT = -5    /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
 } tmd_status;
 
-/* Limits: n_attached + n_unattached < 2^32; trk_ncl in [1, 65535]; n_rows <= 255; n_az <= 63; n_sides in {1,2};
+#define TMD_MAX_CLUSTERS 0xFFFF0000ull /* n_attached + n_unattached <= this (32-bit indices with headroom for tile overshoot) */
+
+/* Limits: n_attached + n_unattached <= TMD_MAX_CLUSTERS; trk_ncl in [1, 65535]; n_rows <= 255; n_az <= 63; n_sides in {1,2};
  * n_sectors_out <= n_az * n_sides; n_sectors_out * n_rows <= 8192. */
 
 /* Pad-plane geometry (DESIGN.md §3 reading 1).  HOST pointers; deep-copied by tmd_create. */

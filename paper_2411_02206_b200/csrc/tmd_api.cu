@@ -100,7 +100,7 @@ __global__ void k_validate(DevGeo G, tmd_compressed in, const uint32_t* __restri
 
 int check_args(const tmd_ctx* ctx, const tmd_compressed* in, const tmd_output* out, bool device_side) {
   if (!ctx || !in || !out) return TMD_ERR_ARG;
-  if (in->n_attached + in->n_unattached >= (1ull << 32)) return TMD_ERR_ARG;
+  if (in->n_attached + in->n_unattached > TMD_MAX_CLUSTERS) return TMD_ERR_ARG;
   if (in->n_attached < in->n_tracks) return TMD_ERR_ARG;
   if ((in->n_tracks == 0) != (in->n_attached == 0)) return TMD_ERR_ARG;
   const bool has_trk = in->n_tracks > 0, has_res = in->n_attached > in->n_tracks, has_un = in->n_unattached > 0;
@@ -207,7 +207,7 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
 
 int tmd_workspace_bytes(const tmd_ctx* ctx, uint32_t n_tracks, uint64_t n_att, uint64_t n_unatt, size_t* out_bytes) {
   if (!ctx || !out_bytes) return TMD_ERR_ARG;
-  if (n_att + n_unatt >= (1ull << 32) || n_att < n_tracks) return TMD_ERR_ARG;
+  if (n_att + n_unatt > TMD_MAX_CLUSTERS || n_att < n_tracks) return TMD_ERR_ARG;
   *out_bytes = layout(ctx->geo.n_bins, n_tracks, n_att).total;
   return TMD_OK;
 }
@@ -365,7 +365,7 @@ int tmd_kernel_times(tmd_ctx* ctx, int max_kernels, const char** names, float* m
 int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compressed* out, void* workspace, size_t workspace_bytes,
                         void* cuda_stream) {
   if (!ctx || !in || !out) return TMD_ERR_ARG;
-  if (in->n_attached >= (1ull << 32) || in->n_attached < in->n_tracks) return TMD_ERR_ARG;
+  if (in->n_attached > TMD_MAX_CLUSTERS || in->n_attached < in->n_tracks) return TMD_ERR_ARG;
   if (in->n_tracks == 0) return in->n_attached == 0 ? TMD_OK : TMD_ERR_ARG;
   if (!in->trk_ncl || !in->trk_qptf || !in->att || !in->leg) return TMD_ERR_ARG;
   void* outs[] = {(void*)out->trk_qpt, (void*)out->trk_row0, (void*)out->trk_sec0, (void*)out->trk_pad0, (void*)out->trk_time0,
