@@ -49,14 +49,19 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
 struct Workspace {
-  uint32_t n_tiles, n_chunks, n_groups;
+  uint32_t n_tiles, n_chunks, n_groups, chunk_shift;
   size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
 };
 
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   Workspace w;
   w.n_tiles = (n_tracks + SCAN_TILE - 1) / SCAN_TILE;
-  w.n_chunks = (uint32_t)((n_att + CHUNK_WINDOW - 1) >> CHUNK_SHIFT);
+  // chunk size: the largest power of two that still leaves about one chunk per resident warp of the rank kernel
+  // (B200: 148 SMs x 20 warps); a pure function of n_att, so tmd_workspace_bytes and tmd_decode agree
+  int shift = CHUNK_SHIFT_MIN;
+  while (shift < CHUNK_SHIFT_MAX && (n_att >> (shift + 1)) >= 2960) ++shift;
+  w.chunk_shift = (uint32_t)shift;
+  w.n_chunks = (uint32_t)((n_att + (1ull << shift) - 1) >> shift);
   w.n_groups = (w.n_chunks + COL_GROUP - 1) / COL_GROUP;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
@@ -283,7 +288,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     TMD_AFTER("track_decode", st);
     // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
     RankArgs R;
-    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att; R.n_chunks = W.n_chunks;
+    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att; R.n_chunks = W.n_chunks; R.chunk_shift = W.chunk_shift;
     uint32_t per_sm = (uint32_t)((size_t)(227 * 1024) / (ctx->rank_smem + 1024));
     if (per_sm < 1) per_sm = 1;
     if (per_sm > 16) per_sm = 16;
@@ -333,7 +338,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     ScatterArgs S;
     S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
     S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
-    S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un;
+    S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un; S.chunk_shift = W.chunk_shift;
     TMD_BEFORE(st);
     k_scatter<<<(n_att + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, 0, st>>>(G, S);
     TMD_AFTER("scatter", st);

@@ -11,11 +11,12 @@
 
 namespace tmd {
 
-// A "chunk" is the set of tracks whose first cluster's global attached index g = off[t] falls in one window of
-// 2^CHUNK_SHIFT clusters.  Chunks are the unit of the deterministic scatter: per-chunk histograms over
-// bins, a column scan over chunks, and ranks inside the chunk.
-constexpr int CHUNK_SHIFT = 15;
-constexpr uint32_t CHUNK_WINDOW = 1u << CHUNK_SHIFT;
+// A "chunk" is a window of 2^chunk_shift consecutive attached clusters (in g order).  Chunks are the unit of the
+// deterministic scatter: per-chunk histograms over bins, a column scan over chunks, and ranks inside the
+// chunk.  The shift is chosen per call from the number of attached clusters (tmd_api.cu): 2^15 for a full time frame,
+// smaller for small inputs so that the rank kernel still has a chunk for every resident warp.
+constexpr int CHUNK_SHIFT_MAX = 15;     // rank16 and the u16 histograms hold counts <= 2^15
+constexpr int CHUNK_SHIFT_MIN = 11;
 constexpr uint32_t MAX_BINS = 8192;     // n_sectors_out * n_rows
 constexpr uint32_t COL_GROUP = 64;      // chunks per group in the column scan
 constexpr uint16_t BIN_INVALID = 0xFFFFu;

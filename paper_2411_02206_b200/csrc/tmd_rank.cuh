@@ -3,9 +3,9 @@
 // the geometry walk of the track-decode kernel (tmd_decode.cuh), which leaves bin(g) in its intermediate records.
 //
 // Together with the column scan (tmd_scan.cuh) this yields the canonical position of every attached cluster
-// (DESIGN.md §3 reading 11):   position(g) = rel[g >> CHUNK_SHIFT][bin(g)] + rank16[g].
+// (DESIGN.md §3 reading 11):   position(g) = rel[g >> chunk_shift][bin(g)] + rank16[g].
 //
-// Design: ONE WARP owns one chunk of 32768 consecutive clusters and goes through it in g order, 32 clusters at a time.
+// Design: ONE WARP owns one chunk of 2^chunk_shift (32768 for a full time frame) consecutive clusters and goes through it in g order, 32 clusters at a time.
 // Because a warp executes in order, the rank is a plain read-increment of a per-warp counter array in shared memory --
 // no atomics, no sort, and the result is the sequential one by construction.  The 32 clusters are cut into runs of
 // strictly ascending (or descending) bins, inside which all bins differ, so one conflict-free load / store round serves
@@ -26,7 +26,7 @@ struct RankArgs {
   const uint2* inter;           // [n_attached] intermediate records of the track-decode kernel; bin = .y >> 16
   uint16_t* hist;               // [n_chunks][n_bins]
   uint16_t* rank16;             // [n_attached]
-  uint32_t n_attached, n_chunks;
+  uint32_t n_attached, n_chunks, chunk_shift;
 };
 
 // bytes of dynamic shared memory per warp: cnt u16[n_bins], padded to 16 bytes
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(WR_THREADS) k_rank(DevGeo G, RankArgs A) {
   uint16_t* cnt = reinterpret_cast<uint16_t*>(smem_raw + (size_t)wib * cnt_bytes);
   const uint32_t n_warps = gridDim.x * WR_WARPS;
   for (uint32_t c = blockIdx.x * WR_WARPS + wib; c < A.n_chunks; c += n_warps) {
-    const uint32_t g0 = c << CHUNK_SHIFT, g1 = min(g0 + CHUNK_WINDOW, A.n_attached);
+    const uint32_t g0 = c << A.chunk_shift, g1 = min(g0 + (1u << A.chunk_shift), A.n_attached);
     __syncwarp();
     for (uint32_t i = lane; i < cnt_bytes / 16; i += 32) reinterpret_cast<uint4*>(cnt)[i] = make_uint4(0, 0, 0, 0);
     __syncwarp();
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(WR_THREADS) k_rank(DevGeo G, RankArgs A) {
     }
     __syncwarp();
     uint16_t* hist_row = A.hist + (size_t)c * n_bins;
-    for (uint32_t b = lane; b < n_bins; b += 32) hist_row[b] = cnt[b];   // <= CHUNK_WINDOW = 32768
+    for (uint32_t b = lane; b < n_bins; b += 32) hist_row[b] = cnt[b];   // <= 2^CHUNK_SHIFT_MAX = 32768
   }
 }
 

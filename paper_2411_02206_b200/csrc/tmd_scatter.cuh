@@ -1,6 +1,6 @@
 // tmd_scatter.cuh -- A6: copy-through of the charge / width / flag fields and the deterministic scatter of the attached
 // clusters into canonical order (DESIGN.md §3 reading 11):
-//   position(g) = rel[g >> CHUNK_SHIFT][bin(g)] + rank16[g]
+//   position(g) = rel[g >> chunk_shift][bin(g)] + rank16[g]
 // with bin(g), T, P from the track-decode kernel's intermediate record, rank16 from the rank kernel (tmd_rank.cuh) and
 // rel from the column scan (tmd_scan.cuh).  Integer / byte moves only.
 //
@@ -23,7 +23,7 @@ struct ScatterArgs {
   const uint32_t* rel;      // [n_chunks][n_bins]
   const uint16_t* a_qtot; const uint16_t* a_qmax; const uint8_t* a_flags; const uint8_t* a_sigpad; const uint8_t* a_sigtime;
   uint4* clusters;
-  uint32_t n_attached, n_clusters_total;
+  uint32_t n_attached, n_clusters_total, chunk_shift;
 };
 
 constexpr int SCATTER_THREADS = 256;
@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(SCATTER_THREADS) k_scatter(DevGeo G, ScatterAr
   const uint32_t sigpad = __ldg(A.a_sigpad + g), sigtime = __ldg(A.a_sigtime + g), flags = __ldg(A.a_flags + g);
   const uint32_t bin = rec.y >> 16;
   if (bin == BIN_INVALID) return;   // decoded sector has no output bin (reading 20)
-  const uint32_t pos = __ldg(A.rel + (size_t)(g >> CHUNK_SHIFT) * G.n_bins + bin) + rank;
+  const uint32_t pos = __ldg(A.rel + (size_t)(g >> A.chunk_shift) * G.n_bins + bin) + rank;
   const uint32_t sec = (bin * G.rows_magic) >> 24, row = bin - sec * G.n_rows;
   if (pos < A.n_clusters_total) A.clusters[pos] = pack_cluster(rec.x, rec.y & 0xFFFFu, qtot, qmax, sigpad, sigtime, flags, row, sec);
 }
