@@ -39,7 +39,7 @@ struct tmd_ctx {
   } slots[TMD_HOST_SLOTS];
   cudaStream_t s_h2d, s_dec, s_d2h;
   bool host_ready;
-  size_t decode_smem, rank_smem;
+  size_t decode_smem, rank_smem, scatter_smem;
   int n_sm;
 };
 
@@ -50,7 +50,7 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
 struct Workspace {
   uint32_t n_tiles, n_chunks, n_groups, chunk_shift;
-  size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_rel, o_rank16, o_inter, total;
+  size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_start16, o_rel, o_rank16, o_inter, total;
 };
 
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
@@ -73,6 +73,7 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   w.o_u_start = take(((size_t)n_bins + 1) * 4);
   w.o_gsum = take((size_t)w.n_groups * n_bins * 4);
   w.o_hist = take((size_t)w.n_chunks * n_bins * 2);
+  w.o_start16 = take((size_t)w.n_chunks * sc_start_stride(n_bins) * 2);
   w.o_rel = take((size_t)w.n_chunks * n_bins * 4);
   w.o_rank16 = take((size_t)n_att * 2);
   w.o_inter = take((size_t)n_att * 8);
@@ -177,6 +178,9 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   const uint32_t n_bins_c = g->n_sectors_out * g->n_rows;
   ctx->rank_smem = (size_t)WR_WARPS * wr_warp_smem(n_bins_c);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->rank_smem);
+  ctx->scatter_smem = sc_smem_bytes(n_bins_c);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->scatter_smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scatter, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
   ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_track_decode<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
@@ -236,6 +240,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   uint32_t* d_ustart = (uint32_t*)(ws + W.o_u_start);
   uint32_t* d_gsum = (uint32_t*)(ws + W.o_gsum);
   uint16_t* d_hist = (uint16_t*)(ws + W.o_hist);
+  uint16_t* d_start16 = (uint16_t*)(ws + W.o_start16);
   uint32_t* d_rel = (uint32_t*)(ws + W.o_rel);
   uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
   uint2* d_inter = (uint2*)(ws + W.o_inter);
@@ -288,7 +293,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     TMD_AFTER("track_decode", st);
     // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
     RankArgs R;
-    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att; R.n_chunks = W.n_chunks; R.chunk_shift = W.chunk_shift;
+    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att; R.n_chunks = W.n_chunks; R.chunk_shift = W.chunk_shift; R.start16 = d_start16; R.start_stride = sc_start_stride(n_bins);
     uint32_t per_sm = (uint32_t)((size_t)(227 * 1024) / (ctx->rank_smem + 1024));
     if (per_sm < 1) per_sm = 1;
     if (per_sm > 16) per_sm = 16;
@@ -339,8 +344,21 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
     S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
     S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un; S.chunk_shift = W.chunk_shift;
+    S.start16 = d_start16; S.start_stride = sc_start_stride(n_bins);
     TMD_BEFORE(st);
-    k_scatter<<<(n_att + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, 0, st>>>(G, S);
+    {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(W.n_chunks * SC_CLUSTER);
+      cfg.blockDim = dim3(SC_THREADS);
+      cfg.dynamicSmemBytes = ctx->scatter_smem;
+      cfg.stream = st;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = SC_CLUSTER; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+      cfg.attrs = attr;
+      cfg.numAttrs = 1;
+      if (cudaLaunchKernelEx(&cfg, k_scatter, G, S) != cudaSuccess) return TMD_ERR_CUDA;
+    }
     TMD_AFTER("scatter", st);
   }
   if (fork) TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));   // join: everything is ordered before later work on `st`

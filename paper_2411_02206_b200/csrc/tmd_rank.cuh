@@ -26,7 +26,8 @@ struct RankArgs {
   const uint2* inter;           // [n_attached] intermediate records of the track-decode kernel; bin = .y >> 16
   uint16_t* hist;               // [n_chunks][n_bins]
   uint16_t* rank16;             // [n_attached]
-  uint32_t n_attached, n_chunks, chunk_shift;
+  uint16_t* start16;            // [n_chunks][start_stride] exclusive scan of the hist row; entry n_bins = clusters with a bin
+  uint32_t n_attached, n_chunks, chunk_shift, start_stride;
 };
 
 // bytes of dynamic shared memory per warp: cnt u16[n_bins], padded to 16 bytes
@@ -108,6 +109,29 @@ __global__ void __launch_bounds__(WR_THREADS) k_rank(DevGeo G, RankArgs A) {
     __syncwarp();
     uint16_t* hist_row = A.hist + (size_t)c * n_bins;
     for (uint32_t b = lane; b < n_bins; b += 32) hist_row[b] = cnt[b];   // <= 2^CHUNK_SHIFT_MAX = 32768
+    // first slot of every bin in the chunk's (bin, rank) order, for the scatter kernel: lane l scans bins [l*per, l*per+per)
+    {
+      const uint32_t per = (n_bins + 31) / 32, b0 = min(lane * per, n_bins), b1 = min(b0 + per, n_bins);
+      uint32_t s = 0;
+      for (uint32_t b = b0; b < b1; ++b) s += cnt[b];
+      uint32_t inc = s;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t p = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= (uint32_t)o) inc += p;
+      }
+      uint32_t ex = inc - s;
+      uint16_t* start_row = A.start16 + (size_t)c * A.start_stride;
+      __syncwarp();                                                        // the hist row has been read out of cnt
+      for (uint32_t b = b0; b < b1; ++b) {
+        const uint32_t h = cnt[b];
+        cnt[b] = (uint16_t)ex;
+        ex += h;
+      }
+      __syncwarp();
+      for (uint32_t b = lane; b < n_bins; b += 32) start_row[b] = cnt[b];  // coalesced
+      if (lane == 31) start_row[n_bins] = (uint16_t)inc;                   // number of clusters of the chunk that have a bin
+    }
   }
 }
 

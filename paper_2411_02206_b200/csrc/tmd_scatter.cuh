@@ -4,29 +4,31 @@
 // with bin(g), T, P from the track-decode kernel's intermediate record, rank16 from the rank kernel (tmd_rank.cuh) and
 // rel from the column scan (tmd_scan.cuh).  Integer / byte moves only.
 //
-// One thread per attached cluster, in g order: every read is coalesced in g; the only irregular accesses are the rel
-// lookups (one 22 KB row per chunk: L1 / L2) and the 16-byte stores, which the L2 merges into full sectors because
-// neighbouring ranks of a bin are written by neighbouring chunks.
-// Measured on B200: what bounds this kernel is the rate of 16-byte stores that are spread over the whole
-// output (~72 G stores/s), not the bytes in flight -- with sequential store addresses the same kernel runs at 6.2 TB/s.
-// Wider variants (2 or 4 clusters per thread, persistent blocks with register prefetch) widen the window of g that is in
-// flight, which makes the stores less local in time, and were slower.
+// Every input stream is read coalesced in g.  What bounded the first version (one thread per cluster, a 16-byte store
+// each: 3.51 ms at c3) was measured to be the half-sector stores spread over the whole output: with sequential store
+// addresses the same kernel ran at 6.2 TB/s, with whole-sector stores a third faster.  Hence the sort
+// through distributed shared memory below.
 #pragma once
 
+#include <cooperative_groups.h>
+
 #include "tmd_common.cuh"
+#include "tmd_scan.cuh"
 
 namespace tmd {
+
+namespace cg = cooperative_groups;
 
 struct ScatterArgs {
   const uint2* inter;       // [n_attached] {T, P | bin << 16}
   const uint16_t* rank16;   // [n_attached]
   const uint32_t* rel;      // [n_chunks][n_bins]
+  const uint16_t* start16;  // [n_chunks][start_stride] first slot of every bin in the chunk's (bin, rank) order; [n_bins] = total
   const uint16_t* a_qtot; const uint16_t* a_qmax; const uint8_t* a_flags; const uint8_t* a_sigpad; const uint8_t* a_sigtime;
   uint4* clusters;
-  uint32_t n_attached, n_clusters_total, chunk_shift;
+  uint32_t n_attached, n_clusters_total, chunk_shift, start_stride;
 };
 
-constexpr int SCATTER_THREADS = 256;
 
 __device__ __forceinline__ uint4 pack_cluster(uint32_t T, uint32_t P, uint32_t qtot, uint32_t qmax, uint32_t sigpad, uint32_t sigtime,
                                               uint32_t flags, uint32_t row, uint32_t sec) {
@@ -38,17 +40,79 @@ __device__ __forceinline__ uint4 pack_cluster(uint32_t T, uint32_t P, uint32_t q
   return v;
 }
 
-__global__ void __launch_bounds__(SCATTER_THREADS) k_scatter(DevGeo G, ScatterArgs A) {
-  const uint32_t g = blockIdx.x * SCATTER_THREADS + threadIdx.x;
-  if (g >= A.n_attached) return;
-  const uint2 rec = __ldg(A.inter + g);
-  const uint32_t rank = __ldg(A.rank16 + g), qtot = __ldg(A.a_qtot + g), qmax = __ldg(A.a_qmax + g);
-  const uint32_t sigpad = __ldg(A.a_sigpad + g), sigtime = __ldg(A.a_sigtime + g), flags = __ldg(A.a_flags + g);
-  const uint32_t bin = rec.y >> 16;
-  if (bin == BIN_INVALID) return;   // decoded sector has no output bin (reading 20)
-  const uint32_t pos = __ldg(A.rel + (size_t)(g >> A.chunk_shift) * G.n_bins + bin) + rank;
-  const uint32_t sec = (bin * G.rows_magic) >> 24, row = bin - sec * G.n_rows;
-  if (pos < A.n_clusters_total) A.clusters[pos] = pack_cluster(rec.x, rec.y & 0xFFFFu, qtot, qmax, sigpad, sigtime, flags, row, sec);
+// ---- scatter through distributed shared memory -----------------------------------------------------------------------
+// A thread-block cluster of SC_CLUSTER = 16 CTAs owns one chunk.  The chunk's records are first sorted by (bin, rank) INSIDE
+// the cluster: record g goes to slot start[bin] + rank16[g] of a 2^chunk_shift-record array that is spread over the shared
+// memories of the 16 CTAs (start = exclusive scan of the chunk's histogram row, from the rank kernel; the store is a DSMEM store,
+// st.shared::cluster).  After a cluster barrier every CTA writes its part of the sorted array: records of one bin are now
+// neighbours, so the ~6 records a chunk adds to a bin leave as one contiguous piece and most 32-byte sectors are written
+// whole.  Measured: 16-byte stores that fill half a sector are what bounded the one-thread-per-cluster
+// scatter (a partial-sector write is a read-modify-write in the ECC-protected L2).
+constexpr int SC_CLUSTER = 16;                      // non-portable cluster size (needs cudaFuncAttributeNonPortableClusterSizeAllowed)
+constexpr int SC_CLUSTER_SHIFT = 4;
+constexpr int SC_THREADS = 256;
+constexpr int SC_UNROLL = 4;
+constexpr uint32_t SC_MAX_PER_CTA = (1u << CHUNK_SHIFT_MAX) / SC_CLUSTER;   // 2048 records = 32 KB
+
+// row stride (entries) of the start16 table: n_bins + 1 entries, padded to 16 bytes
+__host__ __device__ inline uint32_t sc_start_stride(uint32_t n_bins) { return (n_bins + 1 + 7) & ~7u; }
+__host__ __device__ inline size_t sc_smem_bytes(uint32_t n_bins) { return (size_t)SC_MAX_PER_CTA * 16 + (size_t)sc_start_stride(n_bins) * 2; }
+
+__global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(DevGeo G, ScatterArgs A) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  uint4* recs = reinterpret_cast<uint4*>(smem_raw);                                   // this CTA's part of the sorted chunk
+  uint16_t* start = reinterpret_cast<uint16_t*>(smem_raw + (size_t)SC_MAX_PER_CTA * 16);  // [n_bins + 1] first slot of every bin
+  cg::cluster_group cluster = cg::this_cluster();
+  const uint32_t rank_in_cluster = cluster.block_rank();
+  const uint32_t c = blockIdx.x >> SC_CLUSTER_SHIFT, tid = threadIdx.x, n_bins = G.n_bins;
+  const uint32_t per_shift = A.chunk_shift - SC_CLUSTER_SHIFT, per_cta = 1u << per_shift;
+  // ---- start[bin]: the chunk's row of the table the rank kernel wrote (every CTA keeps a copy)
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(A.start16 + (size_t)c * A.start_stride);
+    for (uint32_t i = tid; i < A.start_stride / 8; i += SC_THREADS) reinterpret_cast<uint4*>(start)[i] = __ldg(src + i);
+  }
+  // ---- this CTA's share of g: loads in flight before the cluster barrier
+  const uint32_t g_base = (c << A.chunk_shift) + (rank_in_cluster << per_shift);
+  bool first = true;
+  for (uint32_t i0 = 0; i0 < per_cta; i0 += SC_THREADS * SC_UNROLL) {
+    uint2 rec[SC_UNROLL];
+    uint32_t rk[SC_UNROLL], qt[SC_UNROLL], qm[SC_UNROLL], sp[SC_UNROLL], st[SC_UNROLL], fl[SC_UNROLL];
+#pragma unroll
+    for (int k = 0; k < SC_UNROLL; ++k) {
+      const uint32_t i = i0 + k * SC_THREADS + tid, g = g_base + i;
+      rec[k] = make_uint2(0u, 0xFFFF0000u);
+      if (i < per_cta && g < A.n_attached) {
+        rec[k] = __ldg(A.inter + g);
+        rk[k] = __ldg(A.rank16 + g); qt[k] = __ldg(A.a_qtot + g); qm[k] = __ldg(A.a_qmax + g);
+        sp[k] = __ldg(A.a_sigpad + g); st[k] = __ldg(A.a_sigtime + g); fl[k] = __ldg(A.a_flags + g);
+      }
+    }
+    if (first) {
+      cluster.sync();                                // start[] visible; every CTA of the cluster is running
+      first = false;
+    }
+#pragma unroll
+    for (int k = 0; k < SC_UNROLL; ++k) {
+      const uint32_t bin = rec[k].y >> 16;
+      if (bin == BIN_INVALID) continue;              // no output bin (reading 20), or past the end
+      const uint32_t sec = (bin * G.rows_magic) >> 24, row = bin - sec * G.n_rows;
+      const uint32_t slot = (uint32_t)start[bin] + rk[k];
+      uint4* remote = cluster.map_shared_rank(recs, slot >> per_shift);
+      remote[slot & (per_cta - 1)] = pack_cluster(rec[k].x, rec[k].y & 0xFFFFu, qt[k], qm[k], sp[k], st[k], fl[k], row, sec);
+    }
+  }
+  cluster.sync();                                    // the sorted chunk is complete
+  // ---- this CTA's part of the sorted chunk to its canonical positions
+  const uint32_t n_valid = start[n_bins];
+  const uint32_t* __restrict__ rel_row = A.rel + (size_t)c * n_bins;
+  for (uint32_t i = tid; i < per_cta; i += SC_THREADS) {
+    const uint32_t p = (rank_in_cluster << per_shift) + i;
+    if (p >= n_valid) break;
+    const uint4 v = recs[i];
+    const uint32_t bin = ((v.w >> 16) & 0xFFu) * G.n_rows + ((v.w >> 8) & 0xFFu);
+    const uint32_t pos = __ldg(rel_row + bin) + (p - (uint32_t)start[bin]);
+    if (pos < A.n_clusters_total) A.clusters[pos] = v;
+  }
 }
 
 }  // namespace tmd
