@@ -105,13 +105,23 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(DevGeo G, ScatterArgs
   // ---- this CTA's part of the sorted chunk to its canonical positions
   const uint32_t n_valid = start[n_bins];
   const uint32_t* __restrict__ rel_row = A.rel + (size_t)c * n_bins;
-  for (uint32_t i = tid; i < per_cta; i += SC_THREADS) {
-    const uint32_t p = (rank_in_cluster << per_shift) + i;
-    if (p >= n_valid) break;
-    const uint4 v = recs[i];
-    const uint32_t bin = ((v.w >> 16) & 0xFFu) * G.n_rows + ((v.w >> 8) & 0xFFu);
-    const uint32_t pos = __ldg(rel_row + bin) + (p - (uint32_t)start[bin]);
-    if (pos < A.n_clusters_total) A.clusters[pos] = v;
+  uint4* __restrict__ out = A.clusters;
+  for (uint32_t i0 = 0; i0 < per_cta; i0 += SC_THREADS * SC_UNROLL) {
+    uint4 v[SC_UNROLL];
+    uint32_t pos[SC_UNROLL];
+#pragma unroll
+    for (int k = 0; k < SC_UNROLL; ++k) {                     // the lookups of the batch in flight together
+      const uint32_t i = i0 + k * SC_THREADS + tid, p = (rank_in_cluster << per_shift) + i;
+      pos[k] = 0xFFFFFFFFu;
+      if (i < per_cta && p < n_valid) {
+        v[k] = recs[i];
+        const uint32_t bin = ((v[k].w >> 16) & 0xFFu) * G.n_rows + ((v[k].w >> 8) & 0xFFu);
+        pos[k] = __ldg(rel_row + bin) + (p - (uint32_t)start[bin]);
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < SC_UNROLL; ++k)
+      if (pos[k] < A.n_clusters_total) out[pos[k]] = v[k];
   }
 }
 
