@@ -66,6 +66,7 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(DevGeo G, ScatterArgs
   const uint32_t rank_in_cluster = cluster.block_rank();
   const uint32_t c = blockIdx.x >> SC_CLUSTER_SHIFT, tid = threadIdx.x, n_bins = G.n_bins;
   const uint32_t per_shift = A.chunk_shift - SC_CLUSTER_SHIFT, per_cta = 1u << per_shift;
+  cluster.barrier_arrive();                          // "this CTA is running": waited for just before the first remote store
   // ---- start[bin]: the chunk's row of the table the rank kernel wrote (every CTA keeps a copy)
   {
     const uint4* src = reinterpret_cast<const uint4*>(A.start16 + (size_t)c * A.start_stride);
@@ -88,7 +89,8 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(DevGeo G, ScatterArgs
       }
     }
     if (first) {
-      cluster.sync();                                // start[] visible; every CTA of the cluster is running
+      __syncthreads();                               // start[] visible
+      cluster.barrier_wait();                        // every CTA of the cluster is running (they arrived before their loads)
       first = false;
     }
 #pragma unroll
