@@ -231,3 +231,28 @@ def test_pipelined_host_entry_points_match():
             T.tmd_decode_host_async(ctx, T.make_compressed(held[0][0]), T.make_output(held[0][1], held[0][2]), T.TMD_VALIDATE, 0)
     finally:
         T.tmd_destroy(ctx)
+
+
+def test_serial_and_timing_flags_do_not_change_the_result():
+    # TMD_SERIAL (one stream) and TMD_TIMING (event pairs around the kernels) are the modes bench.py's per-kernel pass uses
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    geo = build_geometry(36)
+    c = random_compressed(geo, 5000, 60_000, 51, max_ncl=180)
+    want = O.decode(geo, BZ, c)
+    for flags in (T.TMD_SERIAL, T.TMD_TIMING, T.TMD_SERIAL | T.TMD_TIMING, T.TMD_SERIAL | T.TMD_VALIDATE):
+        assert_same(gpu_decode(geo, BZ, c, flags=flags), want)
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        from gpu_util import _as_torch
+        from tmd_inputs.layout import COMPRESSED_FIELDS
+        dev = {k: _as_torch(np.ascontiguousarray(getattr(c, k))).cuda() for k in COMPRESSED_FIELDS}
+        n = c.n_attached + c.n_unattached
+        out = T.make_output(torch.empty(n * 16, dtype=torch.uint8, device="cuda"), torch.empty(geo.n_bins + 1, dtype=torch.int32, device="cuda"),
+                            torch.empty(T.tmd_workspace_bytes(ctx, c.n_tracks, c.n_attached, c.n_unattached), dtype=torch.uint8, device="cuda"))
+        T.tmd_decode(ctx, T.make_compressed(dev), out, T.TMD_TIMING | T.TMD_SERIAL, torch.cuda.current_stream().cuda_stream)
+        times = dict(T.tmd_kernel_times(ctx))
+        assert T.tmd_last_launch_count(ctx) == len(times) == 12
+        assert {"track_decode", "rank", "scatter", "unattached", "bin_offsets"} <= set(times) and all(v >= 0 for v in times.values())
+    finally:
+        T.tmd_destroy(ctx)
