@@ -270,7 +270,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   }
   if (validate) {
     TMD_BEFORE(st);
-    k_validate<<<148, 256, 0, st>>>(G, *in, d_off, d_err);
+    k_validate<<<ctx->n_sm, 256, 0, st>>>(G, *in, d_off, d_err);
     TMD_AFTER("validate", st);
     uint32_t h_err[ERR_WORDS];
     TMD_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
