@@ -20,8 +20,11 @@
  * Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`): worked trace tests/golden/c9_trace.txt; closed forms
  * (straight radial track, mirror twice); noiseless exact helices give residuals of a few codes (physical fidelity:
  * a dropped term / wrong sign / wrong index blows this up); numpy.cumsum / stable argsort for offsets, unattached
- * sums and the canonical order; decode(encode(x)) == x; brute-force checks on tiny inputs.  No function here is
- * "parity unpinned".
+ * sums and the canonical order; decode(encode(x)) == x; brute-force checks on tiny inputs; and, for every branch of
+ * orc_init / orc_step (the `!ok` path, multi-step rotations, the saturation constants, reading 19's reductions), an
+ * independent numpy-float32 evaluation of the op list (tests/c3_numpy.py, tests/test_oracle_independent.py) compared
+ * per step on all 20 trace columns.  DESIGN.md §4 lists mutation -> failing test.  No function here is "parity
+ * unpinned".
  */
 #include <math.h>
 #include <stdint.h>
