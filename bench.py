@@ -2,14 +2,16 @@
 """bench.py -- decoded TPC clusters/s of the track-model decoder on synthetic time frames (BASELINE.json metric).
 
 One "step" = one pass of the whole hot path over one synthetic time frame:
-`tmd_decode` through the C ABI, compressed SoA resident in HBM.  Prints ONE JSON line (see the task contract):
+`tmd_decode(flags = 0)` through the C ABI, compressed SoA resident in HBM.  Prints ONE JSON line (see the task contract):
 value = clusters decoded per second over all ranks (device-timed with CUDA events, max over ranks), `e2e` = the same
-through `tmd_decode_host` with pinned HOST buffers (copies inside the timed region), `roofline` for the dominant kernel
-(timed live with CUDA events the library records on the launching stream), `cpu_baseline` = the CPU oracle on a bounded
-sample of the same workload.
+through `tmd_decode_host_async` with pinned HOST buffers (copies inside the timed region), `roofline` for the dominant
+kernel (timed live, outside the timed region, with CUDA events the library records on the launching stream) with the
+instruction-issue bound beside the HBM bound, `cpu_baseline` = the CPU oracle on a bounded sample of the same workload
+(one core, and all host cores), `other_workloads` = the same step timed on c2, c4 and a batch of 64 c1 frames.
 
 Multi-GPU: the path does not shard ("replicas only") -- every rank decodes its own time frame
 (different seed), no collective on the data path; torch.distributed (NCCL) is used for the barrier and the max.
+`python bench.py --gpus N` outside torchrun starts the N ranks itself (torch.distributed.run on 127.0.0.1).
 
 `--impl reference` times the CPU oracle (oracle/, as it stands, single thread) on bounded samples of the same workload.
 """
@@ -18,9 +20,9 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
-import tempfile
 import time
 
 import numpy as np
@@ -31,6 +33,7 @@ sys.path.insert(0, ROOT)
 BZ = 0.5
 METRIC = "decoded_tpc_clusters_per_second"
 UNIT = "clusters/s"
+BATCH_FRAMES = 64          # other_workloads["c1x64"]: SURVEY.md §8(f)-4, many small frames in one call
 
 
 def algorithmic_bytes_attached(n_trk: int, n_att: int) -> int:
@@ -45,7 +48,7 @@ def algorithmic_bytes_unattached(n_un: int, n_bins: int) -> int:
 def kernel_algorithmic_bytes(n_trk: int, n_att: int, n_un: int, n_bins: int) -> dict:
     """The share of the algorithmic bytes each kernel is there to move: the decode kernel consumes the
     per-track fields and the four residual streams, the scatter kernel the copy-through fields and writes the records,
-    the unattached kernel its 13 B in / 16 B out.  The walk/rank and scan kernels move no algorithmic byte (overhead)."""
+    the unattached kernel its 13 B in / 16 B out.  The rank and scan kernels move no algorithmic byte (overhead)."""
     return {"track_decode": 11 * n_trk + 8 * (n_att - n_trk), "scatter": 7 * n_att + 16 * n_att,
             "unattached": algorithmic_bytes_unattached(n_un, n_bins)}
 
@@ -90,7 +93,6 @@ def oracle_sample(workload: str, n_s: int, device):
     """A bounded sample of `workload` for the CPU oracle: the first n_s tracks of the same generator recipe (same pT / length /
     looper mix) and the same fraction of the unattached clusters.  The attached clusters are ENCODED BY THE ORACLE'S OWN
     ENCODER -- nothing the oracle reads comes from the CUDA path."""
-    import torch
     from tmd_inputs import build_geometry, physical as ph, timeframe as tf
     from tmd_inputs.layout import COMPRESSED_FIELDS, Compressed
     from oracle import tmd_oracle as O
@@ -121,15 +123,70 @@ def time_oracle(geo, comp) -> float:
     return time.perf_counter() - t0
 
 
-def cpu_baseline(workload: str, n_s: int, device) -> dict:
+def host_description() -> dict:
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count()}
+
+
+def oracle_all_cores(geo, comp, seconds: float = 4.0) -> dict | None:
+    """The same oracle on ALL host cores: one process per core, each decoding the same bounded sample repeatedly for about
+    `seconds` ("one B200 = N_eq host cores").  Independent processes = independent time frames, which is
+    how the path scales on a CPU farm (PAPER.md L70 compares one GPU with N EPN cores)."""
+    import tempfile
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    n_proc = os.cpu_count() or 1
+    one = time_oracle(geo, comp)
+    reps = max(1, int(seconds / max(one, 1e-3)))
+    with tempfile.TemporaryDirectory(dir="/dev/shm" if os.path.isdir("/dev/shm") else None) as d:
+        np.savez(os.path.join(d, "sample.npz"), **{k: getattr(comp, k) for k in COMPRESSED_FIELDS})
+        cmd = [sys.executable, os.path.abspath(__file__), "--oracle-worker", os.path.join(d, "sample.npz"), "--oracle-reps", str(reps)]
+        procs = [subprocess.Popen(cmd, stdout=subprocess.PIPE, text=True) for _ in range(n_proc)]
+        spans = []
+        for p in procs:
+            out, _ = p.communicate(timeout=600)
+            if p.returncode != 0:
+                return None
+            t0, t1 = (float(v) for v in out.strip().split()[-2:])
+            spans.append((t0, t1))
+    wall = max(t1 for _, t1 in spans) - min(t0 for t0, _ in spans)      # time.time() stamps: first start to last end
+    n_cl = comp.n_attached + comp.n_unattached
+    return {"processes": n_proc, "value": n_proc * reps * n_cl / wall, "unit": UNIT, "reps_per_process": reps}
+
+
+def oracle_worker(path: str, reps: int) -> None:
+    from tmd_inputs import build_geometry
+    from tmd_inputs.layout import Compressed
+    z = np.load(path)
+    comp = Compressed(**{k: z[k] for k in z.files})
+    geo = build_geometry(36)
+    time_oracle(geo, comp)                       # builds / loads liborc.so, touches the pages
+    t0 = time.time()
+    for _ in range(reps):
+        time_oracle(geo, comp)
+    print(t0, time.time())
+
+
+def cpu_baseline(workload: str, n_s: int, device, gpu_value: float, all_cores: bool) -> dict:
     """The oracle as it stands (single thread) timed on a bounded sample of the workload (about 10 s of decoding at c3)."""
     geo, comp, n_s = oracle_sample(workload, n_s, device)
     dt = time_oracle(geo, comp)
     n_cl = comp.n_attached + comp.n_unattached
-    return {"value": n_cl / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"{n_s} tracks of the {workload} recipe ({comp.n_attached} attached) + the same fraction of the unattached "
-                      f"clusters ({comp.n_unattached}), encoded by the oracle encoder; oracle/tmd_oracle.c orc_decode, single "
-                      f"thread, {dt:.2f} s"}
+    out = {"value": n_cl / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"{n_s} tracks of the {workload} recipe ({comp.n_attached} attached) + the same fraction of the unattached "
+                     f"clusters ({comp.n_unattached}), encoded by the oracle encoder; oracle/tmd_oracle.c orc_decode, single "
+                     f"thread, {dt:.2f} s",
+           "host": host_description(), "gpu_equals_host_cores": gpu_value / (n_cl / dt)}
+    if all_cores:
+        small = oracle_sample(workload, max(1000, n_s // 100), device)
+        out["all_cores"] = oracle_all_cores(small[0], small[1])
+    return out
 
 
 # ------------------------------------------------------------------------------------------------ clocks
@@ -183,7 +240,7 @@ class ClockSampler:
                 "power_w_max": max(power)}
 
 
-# ------------------------------------------------------------------------------------------------ arms
+# ------------------------------------------------------------------------------------------------ ranks
 def aggregate_over_ranks(total_ms: float, n_units: float, device):
     """Replicas only: every rank decodes its own time frame.  The job's time is the MAX over ranks of the
     device time, its work the SUM of the units; no collective on the data path.  Works on any backend (NCCL on GPUs,
@@ -203,6 +260,154 @@ def rank_seed_offset(rank: int) -> int:
     return rank
 
 
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(n: int, argv: list[str]) -> int:
+    """`python bench.py --gpus N` outside torchrun: start the N ranks (one per GPU) the way the driver does."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(free_port()), os.path.abspath(__file__), *argv]
+    return subprocess.call(cmd)
+
+
+def run_rank_logic_only(args) -> None:
+    """The multi-rank plumbing of run_ours without a GPU (gloo): which frame a rank takes, max of times, sum of clusters.
+    Used by tests/test_multi_rank.py through `bench.py --gpus 2 --rank-logic-only`."""
+    import torch
+    import torch.distributed as dist
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    ms, n = aggregate_over_ranks(10.0 + 5.0 * rank, 1000.0 + rank_seed_offset(rank), torch.device("cpu"))
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "n_gpus": world, "ms_per_step": ms, "value": n / (ms * 1e-3), "unit": UNIT,
+                          "scaling": "weak", "rank_logic_only": True}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------ timing helpers
+class Frame:
+    """One time frame resident in HBM with its outputs and workspace."""
+
+    def __init__(self, T, ctx, geo, arrays, device):
+        import torch
+        self.arrays = arrays
+        self.n_trk, self.n_att, self.n_un = (int(arrays[k].shape[0]) for k in ("trk_ncl", "a_qtot", "u_qtot"))
+        self.n_cl, self.n_bins = self.n_att + self.n_un, geo.n_bins
+        self.clusters = torch.empty(max(self.n_cl, 1) * 16, dtype=torch.uint8, device=device)
+        self.bin_offset = torch.empty(geo.n_bins + 1, dtype=torch.int32, device=device)
+        self.ws = torch.empty(T.tmd_workspace_bytes(ctx, self.n_trk, self.n_att, self.n_un), dtype=torch.uint8, device=device)
+        self.comp = T.make_compressed(arrays)
+        self.out = T.make_output(self.clusters, self.bin_offset, self.ws)
+
+    def algorithmic_bytes(self) -> int:
+        return algorithmic_bytes_attached(self.n_trk, self.n_att) + algorithmic_bytes_unattached(self.n_un, self.n_bins)
+
+
+def timed_steps(step, steps: int, warmup: int, barrier) -> list[float]:
+    """W untimed calls of `step`, then K timed ones, one CUDA-event pair per step on torch's current stream (the stream the
+    library launches on), bracketed by barrier + synchronize on both sides.  Returns the K per-step times in ms."""
+    import torch
+    for _ in range(warmup):
+        step()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for s0, s1 in ev:
+        s0.record()
+        step()
+        s1.record()
+    barrier()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def per_kernel_ms(T, ctx, frame: Frame, stream, n: int = 3) -> dict:
+    """OUTSIDE the timed region: the same step with an event pair around every kernel (TMD_TIMING), averaged over n runs."""
+    import torch
+    acc: dict[str, float] = {}
+    for _ in range(n):
+        T.tmd_decode(ctx, frame.comp, frame.out, T.TMD_TIMING, stream)
+        for name, ms in T.tmd_kernel_times(ctx):
+            acc[name] = acc.get(name, 0.0) + ms / n
+    torch.cuda.synchronize()
+    return acc
+
+
+def stats(ms: list[float]) -> dict:
+    return {"mean": float(np.mean(ms)), "median": float(np.median(ms)), "min": float(np.min(ms))}
+
+
+def side_workload(T, name: str, device, steps: int, peak: float) -> dict:
+    """ms/step, clusters/s and path fraction of another BASELINE.json config, measured like the main one (single rank)."""
+    import torch
+    geo, arrays = build_workload(name, device)
+    ctx = T.tmd_create(geo, BZ)
+    fr = Frame(T, ctx, geo, arrays, device)
+    stream = torch.cuda.current_stream().cuda_stream
+    ms = timed_steps(lambda: T.tmd_decode(ctx, fr.comp, fr.out, 0, stream), steps, 3, torch.cuda.synchronize)
+    kms = per_kernel_ms(T, ctx, fr, stream)
+    T.tmd_destroy(ctx)
+    st = stats(ms)
+    gbs = fr.algorithmic_bytes() / (st["mean"] * 1e-3) / 1e9
+    return {"n_tracks": fr.n_trk, "n_attached": fr.n_att, "n_unattached": fr.n_un, "steps": steps, "ms_per_step": st["mean"],
+            "ms_per_step_median": st["median"], "ms_per_step_min": st["min"], "value": fr.n_cl / (st["mean"] * 1e-3), "unit": UNIT,
+            "path_gbs": gbs, "path_frac_of_hbm_peak": gbs / peak, "kernel_ms": kms,
+            "l2": "inputs larger than L2, no flush" if fr.algorithmic_bytes() > 400e6 else "L2-resident workload (flag)"}
+
+
+def batch_workload(T, device, n_frames: int, steps: int, peak: float) -> dict | None:
+    """n_frames c1-sized frames (single Pb-Pb-like events, different seeds) decoded by ONE
+    tmd_decode_batch call, next to the same frames decoded one tmd_decode call after the other."""
+    import torch
+    if not hasattr(T, "tmd_decode_batch"):
+        return None
+    frames, geo = [], None
+    ctx = None
+    for i in range(n_frames):
+        geo, arrays = build_workload("c1", device, seed_offset=i)
+        if ctx is None:
+            ctx = T.tmd_create(geo, BZ)
+        frames.append(Frame(T, ctx, geo, arrays, device))
+    stream = torch.cuda.current_stream().cuda_stream
+    comps, outs = [f.comp for f in frames], [f.out for f in frames]
+    batch = T.make_batch(comps, outs)
+    ms_b = timed_steps(lambda: T.tmd_decode_batch(ctx, batch, 0, stream), steps, 3, torch.cuda.synchronize)
+
+    def one_by_one():
+        for c, o in zip(comps, outs):
+            T.tmd_decode(ctx, c, o, 0, stream)
+    ms_s = timed_steps(one_by_one, steps, 3, torch.cuda.synchronize)
+    ms_1 = timed_steps(lambda: T.tmd_decode(ctx, comps[0], outs[0], 0, stream), steps, 3, torch.cuda.synchronize)
+    T.tmd_destroy(ctx)
+    n_cl = sum(f.n_cl for f in frames)
+    alg = sum(f.algorithmic_bytes() for f in frames)
+    sb, ss, s1 = stats(ms_b), stats(ms_s), stats(ms_1)
+    return {"frames": n_frames, "clusters": n_cl, "steps": steps, "ms_per_step": sb["mean"], "ms_per_step_median": sb["median"],
+            "ms_per_step_min": sb["min"], "value": n_cl / (sb["mean"] * 1e-3), "unit": UNIT,
+            "path_gbs": alg / (sb["mean"] * 1e-3) / 1e9, "path_frac_of_hbm_peak": alg / (sb["mean"] * 1e-3) / 1e9 / peak,
+            "same_frames_one_call_each": {"ms": ss["mean"], "value": n_cl / (ss["mean"] * 1e-3)},
+            "single_c1_frame": {"ms": s1["mean"], "value": frames[0].n_cl / (s1["mean"] * 1e-3)},
+            "l2": "each frame is L2-sized; 64 frames = 3 GB of traffic per step, no flush"}
+
+
+def ncu_profile_numbers(kernel: str, workload: str):
+    """(dram bytes per launch, warp instructions per launch, source file) of `kernel` from the committed ncu summary
+    (profiles/traffic.txt: workload kernel dram_bytes warp_inst), else (None, None, None)."""
+    path = os.path.join(ROOT, "profiles", "traffic.txt")
+    try:
+        for line in open(path):
+            v = line.split()
+            if len(v) >= 3 and v[0] == workload and v[1] == kernel:
+                return float(v[2]), (float(v[3]) if len(v) >= 4 else None), "profiles/traffic.txt"
+    except OSError:
+        pass
+    return None, None, None
+
+
+# ------------------------------------------------------------------------------------------------ arms
 def run_ours(args) -> None:
     import torch
     import torch.distributed as dist
@@ -211,20 +416,17 @@ def run_ours(args) -> None:
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     torch.cuda.set_device(local)
     device = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
 
     geo, arrays = build_workload(args.workload, device, seed_offset=rank_seed_offset(rank))
-    n_trk, n_att, n_un = (int(arrays[k].shape[0]) for k in ("trk_ncl", "a_qtot", "u_qtot"))
-    n_cl = n_att + n_un
     ctx = T.tmd_create(geo, BZ)
-    clusters = torch.empty(n_cl * 16, dtype=torch.uint8, device=device)
-    bin_offset = torch.empty(geo.n_bins + 1, dtype=torch.int32, device=device)
-    ws = torch.empty(T.tmd_workspace_bytes(ctx, n_trk, n_att, n_un), dtype=torch.uint8, device=device)
-    comp = T.make_compressed(arrays)
-    out = T.make_output(clusters, bin_offset, ws)
+    fr = Frame(T, ctx, geo, arrays, device)
+    n_trk, n_att, n_un, n_cl = fr.n_trk, fr.n_att, fr.n_un, fr.n_cl
     stream = torch.cuda.current_stream().cuda_stream
 
     def barrier():
@@ -232,42 +434,27 @@ def run_ours(args) -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- the timed region: K production calls (flags = 0), nothing else
     for _ in range(args.warmup):
-        T.tmd_decode(ctx, comp, out, 0, stream)
+        T.tmd_decode(ctx, fr.comp, fr.out, 0, stream)
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    ktimes: dict[str, float] = {}
-    launches = 0
-    for s0, s1 in ev:
-        s0.record()
-        T.tmd_decode(ctx, comp, out, T.TMD_TIMING, stream)
-        s1.record()
-        launches += T.tmd_last_launch_count(ctx)
-        for name, ms in T.tmd_kernel_times(ctx):          # waits for this step's last kernel
-            ktimes[name] = ktimes.get(name, 0.0) + ms
-    barrier()
+    step_ms = timed_steps(lambda: T.tmd_decode(ctx, fr.comp, fr.out, 0, stream), args.steps, 0, barrier)
     clocks = sampler.stop() if sampler else None
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
-    total_ms, n_cl_all = aggregate_over_ranks(total_ms, float(n_cl), device)
+    launches = T.tmd_last_launch_count(ctx) * args.steps
+    total_ms, n_cl_all = aggregate_over_ranks(sum(step_ms), float(n_cl), device)
     ms_per_step = total_ms / args.steps
     value = n_cl_all / (ms_per_step * 1e-3)
-    # ---- outside the timed region: the same step with every kernel alone on one stream (TMD_SERIAL), for the
-    #      per-kernel times without overlap that the roofline of the dominant kernel is computed from
-    kserial: dict[str, float] = {}
-    n_serial = 3
-    for _ in range(n_serial):
-        T.tmd_decode(ctx, comp, out, T.TMD_TIMING | T.TMD_SERIAL, stream)
-        for name, ms in T.tmd_kernel_times(ctx):
-            kserial[name] = kserial.get(name, 0.0) + ms / n_serial
-    torch.cuda.synchronize()
+    # ---- outside the timed region: per-kernel times (event pair around every kernel) for the roofline of the dominant kernel
+    kms = per_kernel_ms(T, ctx, fr, stream)
 
     # ---- end to end: pinned host buffers in, pinned host buffers out, every copy inside the timed region.  Frames go
     #      through the library's two-slot pipeline (tmd_decode_host_async): the upload of frame i+1 runs beside the
     #      download of frame i, as in the paper's deployment; each slot has its own output buffers.
     h_in = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True).copy_(v) for k, v in arrays.items()}
     h2d = sum(v.numel() * v.element_size() for v in h_in.values())
-    del clusters, ws
+    alg_total = fr.algorithmic_bytes()
+    del fr, arrays
     torch.cuda.empty_cache()
     hcomp = T.make_compressed(h_in)
     houts, keep = [], []
@@ -297,6 +484,9 @@ def run_ours(args) -> None:
     t0 = time.perf_counter()
     T.tmd_decode_host(ctx, hcomp, houts[0], 0, stream)
     e2e_single_s = time.perf_counter() - t0
+    T.tmd_destroy(ctx)
+    del h_in, keep, houts, hcomp
+    torch.cuda.empty_cache()
 
     if rank == 0:
         peaks = {}
@@ -305,52 +495,57 @@ def run_ours(args) -> None:
         except OSError:
             pass
         peak, peak_src = (float(peaks["hbm_gbs"]), "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
-        kavg = {k: v / args.steps for k, v in ktimes.items()}
         kalg = kernel_algorithmic_bytes(n_trk, n_att, n_un, geo.n_bins)
-        dom = max(kserial, key=kserial.get)
+        dom = max(kms, key=kms.get)
         alg = kalg.get(dom)
-        achieved = alg / (kserial[dom] * 1e-3) / 1e9 if alg else None
+        achieved = alg / (kms[dom] * 1e-3) / 1e9 if alg else None
+        traffic, warp_inst, src = ncu_profile_numbers(dom, args.workload)
+        # second bound: instruction issue.  One warp instruction per scheduler and cycle, 4 schedulers per SM.
+        props = torch.cuda.get_device_properties(device)
+        sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
+        issue_peak = props.multi_processor_count * 4 * sm_mhz * 1e6
+        second = None
+        if warp_inst:
+            second = {"kind": "issue", "warp_inst": warp_inst, "peak_inst_per_s": issue_peak, "sm_mhz": sm_mhz,
+                      "floor_ms": 1e3 * warp_inst / issue_peak, "frac": warp_inst / (kms[dom] * 1e-3) / issue_peak,
+                      "source": src}
         roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                    "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(dom, args.workload),
-                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kserial[dom],
-                    "kernel_ms_in_timed_region": kavg.get(dom),
-                    "note": "kernel timed alone on one stream (TMD_SERIAL pass after the timed region); in the timed region "
-                            "it shares the GPU with the unattached kernel of the second stream"}
-        total_alg = algorithmic_bytes_attached(n_trk, n_att) + algorithmic_bytes_unattached(n_un, geo.n_bins)
+                    "frac": achieved / peak if achieved else None, "traffic": traffic, "traffic_source": src,
+                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kms[dom], "second_bound": second,
+                    "note": "kernel timed with an event pair around it in a separate pass after the timed region (same stream, "
+                            "same launch configuration)"}
+        st = stats(step_ms)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic",
+            "ms_per_step": ms_per_step, "ms_per_step_median": st["median"], "ms_per_step_min": st["min"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "n_tracks": n_trk, "n_attached": n_att, "n_unattached": n_un,
                        "sectors_x_rows": "36x152", "bz_tesla": BZ, "l2": "inputs larger than L2, no flush"
-                       if total_alg > 400e6 else "L2-resident workload (flag)", "parallelism": f"replicas x{world}"},
+                       if alg_total > 400e6 else "L2-resident workload (flag)", "parallelism": f"replicas x{world}"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
                     "mode": "two-slot pipeline, tmd_decode_host_async", "single_frame_ms": 1e3 * e2e_single_s},
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": roofline,
-            "path_gbs": total_alg / (ms_per_step * 1e-3) / 1e9, "path_frac_of_hbm_peak": total_alg / (ms_per_step * 1e-3) / 1e9 / peak,
-            "kernel_ms": kavg, "kernel_ms_serial": kserial,
-            "kernel_gbs_serial": {k: kalg[k] / (kserial[k] * 1e-3) / 1e9 for k in kalg if k in kserial},
+            "path_gbs": alg_total / (ms_per_step * 1e-3) / 1e9, "path_frac_of_hbm_peak": alg_total / (ms_per_step * 1e-3) / 1e9 / peak,
+            "kernel_ms": kms,
+            "kernel_gbs": {k: kalg[k] / (kms[k] * 1e-3) / 1e9 for k in kalg if k in kms},
         }
+        if world == 1 and not args.no_extras:
+            other = {}
+            for name in ("c2", "c4"):
+                if name != args.workload:
+                    other[name] = side_workload(T, name, device, min(args.steps, 10), peak)
+                    torch.cuda.empty_cache()
+            b = batch_workload(T, device, BATCH_FRAMES, min(args.steps, 10), peak)
+            if b:
+                other[f"c1x{BATCH_FRAMES}"] = b
+            line["other_workloads"] = other
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_tracks, device)
+            line["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_tracks, device, value, not args.no_extras)
         print(json.dumps(line), flush=True)
-    T.tmd_destroy(ctx)
     if world > 1:
         dist.destroy_process_group()
-
-
-def ncu_traffic(kernel: str, workload: str):
-    """dram bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.txt), else None."""
-    try:
-        for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
-            v = line.split()
-            if len(v) >= 3 and v[0] == workload and v[1] == kernel:
-                return float(v[2])
-    except OSError:
-        pass
-    return None
 
 
 def run_reference(args) -> None:
@@ -372,7 +567,7 @@ def run_reference(args) -> None:
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(dts) / len(dts), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "sectors_x_rows": "36x152", "bz_tesla": BZ},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "host": host_description()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }), flush=True)
 
@@ -389,8 +584,19 @@ def main() -> None:
     ap.add_argument("--ref-tracks", type=int, default=25_000, help="tracks per step of the --impl reference arm")
     ap.add_argument("--cpu-tracks", type=int, default=1_000_000, help="tracks of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip other_workloads (c2, c4, 64 x c1) and the all-cores oracle run")
+    ap.add_argument("--rank-logic-only", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--oracle-worker", default=None, help=argparse.SUPPRESS)
+    ap.add_argument("--oracle-reps", type=int, default=1, help=argparse.SUPPRESS)
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.oracle_worker:
+        oracle_worker(args.oracle_worker, args.oracle_reps)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(spawn_ranks(args.gpus, sys.argv[1:]))
+    if args.rank_logic_only:
+        run_rank_logic_only(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -112,3 +112,106 @@ def test_full_time_frame(name):
             assert np.array_equal(rec[f], d[key]), f"track {t}: {f}"
         for f in ("qtot", "qmax", "sigpad", "sigtime", "flags"):
             assert np.array_equal(rec[f], att[f]), f"track {t}: {f}"
+
+
+# ------------------------------------------------------------------------------------------------ the full oracle at full size
+def _host_gb_available() -> float:
+    import psutil
+    return psutil.virtual_memory().available / 2 ** 30
+
+
+def _upload(comp):
+    from gpu_util import _as_torch
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    return {k: _as_torch(np.ascontiguousarray(getattr(comp, k))).cuda() for k in COMPRESSED_FIELDS}
+
+
+def _compare_with_oracle(geo, comp, tag):
+    """tmd_decode in the launch configuration bench.py times (flags 0, no probes) against orc_decode: every record."""
+    from oracle import tmd_oracle as O
+    from tmd_inputs.layout import CLUSTER_DTYPE
+    got, got_bo = _decode_like_bench(geo, _upload(comp))
+    want, want_bo, _ = O.decode(geo, BZ, comp)
+    assert np.array_equal(got_bo.cpu().numpy().view(np.uint32), want_bo), f"{tag}: bin_offset"
+    got = got.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1)
+    if got.tobytes() != want.tobytes():
+        for f in want.dtype.names:
+            bad = np.nonzero(got[f] != want[f])[0]
+            assert bad.size == 0, f"{tag}: {bad.size} records differ in {f}; first at {int(bad[0])}: got {got[f][bad[0]]} want {want[f][bad[0]]}"
+        raise AssertionError(f"{tag}: bytes differ")
+
+
+# host memory the oracle side needs (truth + compressed SoA + two outputs), GB
+@pytest.mark.parametrize("name,need_gb", [("c2", 8), ("c3", 30), ("c4", 14)])
+def test_full_time_frame_against_the_full_oracle(name, need_gb):
+    """BASELINE.json north_star: "bit-exact agreement with the CPU oracle on all five configs".  The whole frame (attached
+    AND unattached clusters) goes through the ORACLE ENCODER (configs: "encoded by the oracle encoder"), tmd_decode runs as
+    bench.py runs it, and every output record and bin offset is compared with orc_decode.  The GPU encoder is compared
+    with the oracle's bytes on the way (it is what builds bench.py's timed workload)."""
+    import torch
+    from oracle import tmd_oracle as O
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs import build_geometry, timeframe as tf
+    from tmd_inputs.layout import CLUSTER_DTYPE
+
+    if _host_gb_available() < need_gb:
+        pytest.skip(f"needs {need_gb} GB of host memory for the oracle side, {_host_gb_available():.0f} GB available")
+    dev = torch.device("cuda", 0)
+    geo = build_geometry(36)
+    mk, n_un, single = tf.WORKLOADS[name]
+    cfg = mk()
+    truth = tf.generate_truth(cfg, geo, dev, batch=2_000_000)
+    un = tf.generate_unattached_truth(geo, n_un, cfg.seed, dev, "inv_x", single)
+    comp = O.encode(geo, BZ, truth.trk_ncl.cpu().numpy().view(np.uint16), truth.trk_qptf.cpu().numpy(),
+                    truth.att.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1), truth.leg.cpu().numpy(),
+                    un.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1))
+    del un
+    # the library's encoder on the same truth: the oracle encoder's bytes
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        tdt = {"<u2": torch.int16, "i1": torch.int8, "u1": torch.uint8, "<u4": torch.int32}
+        mine = {k: torch.zeros(len(getattr(comp, k)), dtype=tdt[dt], device=dev) for k, dt in T.COMPRESSED_ARRAYS
+                if k.startswith(("trk_", "a_")) and k != "trk_ncl"}
+        ws = torch.empty(T.tmd_workspace_bytes(ctx, truth.n_tracks, truth.n_attached, 0), dtype=torch.uint8, device=dev)
+        T.tmd_encode_attached(ctx, truth.trk_ncl, truth.trk_qptf, truth.att, truth.leg, mine, ws, torch.cuda.current_stream().cuda_stream)
+        for k, v in mine.items():
+            assert np.array_equal(v.cpu().numpy().view(getattr(comp, k).dtype), getattr(comp, k)), f"{name}: GPU encoder, {k}"
+        del mine, ws
+    finally:
+        T.tmd_destroy(ctx)
+    del truth
+    torch.cuda.empty_cache()
+    _compare_with_oracle(geo, comp, name)
+
+
+def test_random_bytes_at_the_full_frame_chunk_size():
+    """>= 97 M attached clusters of random bytes: the library picks chunk_shift = 15 (32768-record chunks, multi-trip loops in
+    the scatter, the multi-run path of the rank kernel on every group) -- the launch configuration of c2..c4, which the small
+    adversarial inputs never reach.  Against the full oracle."""
+    from tmd_inputs import build_geometry
+    from tmd_inputs.adversarial import random_compressed
+    if _host_gb_available() < 12:
+        pytest.skip("needs 12 GB of host memory")
+    geo = build_geometry(36)
+    c = random_compressed(geo, 1_000_000, 3_000_000, seed=61, max_ncl=199)
+    assert c.n_attached >= 97_000_000
+    _compare_with_oracle(geo, c, "random bytes, shift 15")
+
+
+def test_whole_chunks_in_one_bin_at_the_full_frame_chunk_size():
+    """Tracks of 65 535 clusters that never leave their first bin, half of them sharing one bin: whole 32768-record chunks
+    fall into a single bin (u16 histogram / rank / start entries at their limit).  Against the full oracle."""
+    from tmd_inputs import build_geometry
+    from tmd_inputs.adversarial import degenerate_same_bin
+    if _host_gb_available() < 12:
+        pytest.skip("needs 12 GB of host memory")
+    geo = build_geometry(36)
+    ncl = np.full(1500, 65535, np.uint16)
+    ncl[::97] = 1
+    ncl[5::211] = 32769
+    extra = int(97_500_000 - ncl.astype(np.int64).sum())
+    if extra > 0:
+        ncl = np.concatenate((ncl, np.full(extra // 65535 + 1, 65535, np.uint16)))
+    c = degenerate_same_bin(geo, ncl, 62, n_un=10_000)
+    assert c.n_attached >= 97_000_000
+    _compare_with_oracle(geo, c, "one bin, shift 15")

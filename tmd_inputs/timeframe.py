@@ -253,6 +253,31 @@ def generate_unattached(geo: Geometry, n_unattached: int, seed: int, device="cpu
     }
 
 
+def generate_unattached_truth(geo: Geometry, n_unattached: int, seed: int, device="cpu", law: str = "inv_x",
+                              single_event: bool = False) -> torch.Tensor:
+    """Unattached clusters of one time frame in the CLUSTER domain (truth for an encoder; the encoder sorts
+    them per region and stores differences).  Per-bin counts Poisson around the `law` density (total Poisson around
+    n_unattached), pad uniform over the row's pads, time uniform over the time frame (or the event's 500 bins), in NO
+    particular order inside a bin.  Returns int32 [n, 4] = 16-byte cluster records (layout.CLUSTER_DTYPE)."""
+    device = torch.device(device)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(seed * 7919 + 17)
+    n_bins = geo.n_bins
+    w = np.ones(n_bins) if law == "uniform" else np.tile(1.0 / geo.row_x_f64, geo.n_sectors_out)
+    mean = torch.as_tensor(n_unattached * w / w.sum(), dtype=torch.float64, device=device)
+    counts = torch.poisson(mean, generator=gen).to(torch.int64)
+    n = int(counts.sum())
+    bins = torch.repeat_interleave(torch.arange(n_bins, device=device), counts)
+    bins = bins[torch.randperm(n, generator=gen, device=device)]                                # arbitrary order
+    row = bins % geo.n_rows
+    width = torch.as_tensor(geo.row_npads.astype(np.int64) * 64, device=device)[row]
+    pad = (torch.rand(n, generator=gen, device=device, dtype=torch.float64) * width).to(torch.int64)
+    span, base = (500.0 * 64.0, 2000.0 * 64.0) if single_event else (float(TF_NBINS) * 64.0, 0.0)
+    time = (base + torch.rand(n, generator=gen, device=device, dtype=torch.float64) * span).to(torch.int64)
+    qtot, qmax, sigpad, sigtime, flags = _copy_through(gen, n, device)
+    return pack_records(time, pad, qtot, qmax, sigpad, sigtime, flags, row, bins // geo.n_rows)
+
+
 # --- BASELINE.json configs at full size -----------------------------------------------------------------------------
 WORKLOADS = {
     # name: (EventConfig factory, n_unattached, unattached single_event)
