@@ -33,7 +33,8 @@ typedef enum {
   TMD_ERR_ALIGN = -2,     /* a device pointer is not aligned as required                                     */
   TMD_ERR_WORKSPACE = -3, /* workspace missing or smaller than tmd_workspace_bytes()                         */
   TMD_ERR_CUDA = -4,      /* a CUDA runtime call failed (allocation, copy, launch)                           */
-  TMD_ERR_CORRUPT = -5    /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
+  TMD_ERR_CORRUPT = -5,   /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
+  TMD_ERR_DEVICE = -6     /* tmd_create: the device cannot run the kernels (no 16-CTA thread-block clusters)  */
 } tmd_status;
 
 #define TMD_MAX_CLUSTERS 0xFFFF0000ull /* n_attached + n_unattached <= this (32-bit indices with headroom for tile overshoot) */
@@ -131,15 +132,20 @@ typedef struct {
 typedef struct tmd_ctx tmd_ctx;
 
 /* flags of tmd_decode */
-#define TMD_VALIDATE 1u /* check on the device that sum(trk_ncl) == n_attached, sum(u_bin_count) == n_unattached,
-                           every trk_ncl >= 1, trk_row0 < n_rows, trk_sec0 < n_az*n_sides and every decoded sector
-                           < n_sectors_out; synchronises the stream; returns TMD_ERR_CORRUPT on failure.
+#define TMD_VALIDATE 1u /* check on the device that sum(trk_ncl) == n_attached (summed in 64 bits), sum(u_bin_count) ==
+                           n_unattached, every trk_ncl >= 1, trk_row0 < n_rows, trk_sec0 < n_az*n_sides -- BEFORE any decode
+                           work is enqueued: the call synchronises the stream, and returns TMD_ERR_CORRUPT with nothing
+                           decoded if a check fails -- and, after the decode, that every decoded sector is
+                           < n_sectors_out (second synchronisation; TMD_ERR_CORRUPT, the offending clusters dropped).
                            Without it such inputs are undefined except that nothing is written out of bounds
                            of `clusters` for a decoded sector >= n_sectors_out (the cluster is dropped). */
 
-#define TMD_TIMING 2u   /* record a CUDA event pair around every kernel, on the stream it runs on (tmd_kernel_times)      */
-#define TMD_SERIAL 4u   /* run every kernel on `cuda_stream` alone (no second stream): per-kernel times without overlap */
+#define TMD_TIMING 2u   /* record a CUDA event pair around every kernel (tmd_kernel_times).  The first such call on a
+                           context creates the 2 x TMD_MAX_KERNELS events; calls with TMD_TIMING must not run concurrently
+                           on one context */
+#define TMD_SERIAL 4u   /* accepted and ignored: every kernel of a call already runs on `cuda_stream`, one after the other */
 #define TMD_MAX_KERNELS 24
+#define TMD_MAX_BATCH 1024 /* frames per tmd_decode_batch call */
 
 /* Uploads the geometry tables to the current CUDA device.  *out_ctx is set only on success. */
 int tmd_create(const tmd_geometry* geometry, const tmd_field* field, tmd_ctx** out_ctx);
@@ -148,14 +154,27 @@ int tmd_create(const tmd_geometry* geometry, const tmd_field* field, tmd_ctx** o
 int tmd_workspace_bytes(const tmd_ctx* ctx, uint32_t n_tracks, uint64_t n_attached, uint64_t n_unattached, size_t* out_bytes);
 
 /*
- * Decode one time frame (rows A1-A7).  Only enqueues work and returns; no allocation, no host synchronisation and no
- * device-to-host copy unless TMD_VALIDATE is set.  The floating-point track decode (A5) and the scatter (A6) run on
- * `cuda_stream` (a cudaStream_t; null = default stream); the integer side (A3 walk and ranks, A4, A7) runs on a second
- * stream owned by the context, forked from and joined back into `cuda_stream` with events, so for the caller the call
- * behaves like work enqueued on `cuda_stream`: results are valid once that stream has been synchronised.
- * Concurrent calls need distinct contexts and workspaces.
+ * Decode one time frame (rows A1-A7).  Only enqueues kernels on `cuda_stream` (a cudaStream_t; null =
+ * default stream) and returns: no allocation, no host synchronisation and no device-to-host copy unless TMD_VALIDATE
+ * (two synchronisations, see above) or TMD_TIMING (event creation on first use) is set.  All kernels run on that one
+ * stream in order: A1 offsets, A2 length sort, A3 + A5 track decode, A3 ranks, A4 column scan and bin offsets, A7
+ * unattached clusters, A6 scatter.  Results are valid once the stream has been synchronised.
+ * Concurrency: the context is read-only during the call (apart from the launch counter, which every call sets to the
+ * same value), so calls on one context from different streams / host threads are allowed as long as they use different
+ * workspaces and outputs and none of them sets TMD_TIMING.
  */
 int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream);
+
+/*
+ * Decode `n_frames` independent time frames with ONE launch sequence (PAPER.md L70 runs "multiple
+ * instances ... concurrently": small frames -- single events, pp-like frames -- do not fill the GPU one at a time).
+ * `in` / `out` are HOST arrays of n_frames structs holding DEVICE pointers exactly as for tmd_decode; every frame has its
+ * own outputs and its own workspace (>= tmd_workspace_bytes of ITS sizes).  The result of frame i is what
+ * tmd_decode(ctx, &in[i], &out[i], ...) produces.  Every kernel's grid gets a frame coordinate; the per-frame arguments
+ * live in frame 0's workspace for the duration of the call.  1 <= n_frames <= TMD_MAX_BATCH; TMD_VALIDATE is not
+ * accepted (TMD_ERR_ARG): it synchronises.  All frames are checked before anything is enqueued.
+ */
+int tmd_decode_batch(tmd_ctx* ctx, uint32_t n_frames, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream);
 
 /*
  * End-to-end convenience: every pointer in `in` / `out` is a HOST pointer (pinned memory makes the copies asynchronous;
@@ -177,6 +196,18 @@ int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uin
 #define TMD_HOST_SLOTS 2
 int tmd_decode_host_async(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot);
 int tmd_host_wait(tmd_ctx* ctx, int slot);
+
+/*
+ * Self test of the arithmetic the track-decode kernel relies on (every model operation is ONE IEEE-754
+ * binary32 round-to-nearest operation).  The kernel issues the fast sequences of IEEE division and square root without
+ * their per-operation range checks (one merged check per cluster instead) and a fused floor-clamp-convert; this call
+ * compares them on the current device with __fdiv_rn / __fsqrt_rn / floorf + clamp: mismatches[0] = square root over
+ * every binary32 argument in [2^-100, 2^100]; mismatches[1] = division over 2^log2_pairs pseudo-random operand pairs
+ * (dividend magnitude in [2^-40, 2^84], divisor magnitude in [2^-10, 2^80]: the ranges the kernel sends down the fast
+ * path) plus an exhaustive grid of edge mantissas x exponents; mismatches[2] = the floor-clamp conversion over every
+ * binary32 pattern.  All three must be 0.  Synchronous; HOST pointer; log2_pairs <= 40.
+ */
+int tmd_selftest_ieee(uint32_t log2_pairs, uint64_t mismatches[3]);
 
 /* Frees the context and its device tables / buffers.  Null is accepted. */
 int tmd_destroy(tmd_ctx* ctx);

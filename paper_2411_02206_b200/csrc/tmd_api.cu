@@ -19,14 +19,18 @@ struct tmd_ctx {
   DevGeo geo;
   RowGeo* d_rows;
   int device;
+  int n_sm;                    // cudaDevAttrMultiProcessorCount
+  size_t smem_per_sm;          // cudaDevAttrMaxSharedMemoryPerMultiprocessor
+  size_t decode_smem, rank_smem, scatter_smem;
+  // Per-call state.  `launches` is the launch count of the last tmd_decode / tmd_decode_batch (the same for every call
+  // with the same flags and emptiness, so concurrent calls store the same value).  The TMD_TIMING event pairs and the
+  // host-pipeline slots are the only other state a call touches: calls with TMD_TIMING, and the tmd_decode_host* entry
+  // points, must not run concurrently on one context; plain tmd_decode calls on different streams may, with distinct
+  // workspaces.
   int launches;
-  // Second stream of tmd_decode: the unattached clusters (A7) are decoded there while the attached ones are scattered
-  // (A6) on the caller's stream.
-  cudaStream_t side;
-  cudaEvent_t ev_fork, ev_join;
-  // TMD_TIMING: one event pair around every kernel of the last tmd_decode, recorded on the stream it ran on
   cudaEvent_t ev_t0[TMD_MAX_KERNELS], ev_t1[TMD_MAX_KERNELS];
   const char* kernel_names[TMD_MAX_KERNELS];
+  int timed_launches;
   bool events_created, timing_valid;
   // tmd_decode_host / tmd_decode_host_async: TMD_HOST_SLOTS frames in flight, each with its own device arena (inputs,
   // outputs, workspace; grown on demand); host->device copies, decode and device->host copies on three streams so that
@@ -39,8 +43,6 @@ struct tmd_ctx {
   } slots[TMD_HOST_SLOTS];
   cudaStream_t s_h2d, s_dec, s_d2h;
   bool host_ready;
-  size_t decode_smem, rank_smem, scatter_smem;
-  int n_sm;
 };
 
 namespace {
@@ -48,18 +50,19 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) & ~(ALIGN - 1); }
 
-struct Workspace {
-  uint32_t n_tiles, n_chunks, n_groups, chunk_shift;
-  size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_start16, o_rel, o_rank16, o_inter, total;
-};
+// frames per k_store_frames launch: the table travels as a by-value kernel parameter (4 KB parameter space)
+constexpr uint32_t STORE_FRAMES = 8;
+struct FrameChunk { FrameArgs f[STORE_FRAMES]; };
+static_assert(sizeof(FrameChunk) <= 3800, "k_store_frames parameters must fit the 4 KB parameter space");
 
-Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
+Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att, int n_sm) {
   Workspace w;
   w.n_tiles = (n_tracks + SCAN_TILE - 1) / SCAN_TILE;
   // chunk size: the largest power of two that still leaves about one chunk per resident warp of the rank kernel
-  // (B200: 148 SMs x 20 warps); a pure function of n_att, so tmd_workspace_bytes and tmd_decode agree
+  // (20 warps per SM); a pure function of (n_att, SM count), so tmd_workspace_bytes and tmd_decode agree
+  const uint64_t want_chunks = (uint64_t)n_sm * 20;
   int shift = CHUNK_SHIFT_MIN;
-  while (shift < CHUNK_SHIFT_MAX && (n_att >> (shift + 1)) >= 2960) ++shift;
+  while (shift < CHUNK_SHIFT_MAX && (n_att >> (shift + 1)) >= want_chunks) ++shift;
   w.chunk_shift = (uint32_t)shift;
   w.n_chunks = (uint32_t)((n_att + (1ull << shift) - 1) >> shift);
   w.n_groups = (w.n_chunks + COL_GROUP - 1) / COL_GROUP;
@@ -77,30 +80,45 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att) {
   w.o_rel = take((size_t)w.n_chunks * n_bins * 4);
   w.o_rank16 = take((size_t)n_att * 2);
   w.o_inter = take((size_t)n_att * 8);
+  w.o_table = take((size_t)TMD_MAX_BATCH * sizeof(FrameArgs));   // the frame table of a batch lives in frame 0's workspace
   w.total = o;
   return w;
 }
 
 inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
 
+// the frame table of tmd_decode_batch: STORE_FRAMES entries per launch, passed by value
+__global__ void k_store_frames(const __grid_constant__ FrameChunk C, FrameArgs* __restrict__ table, uint32_t first, uint32_t count) {
+  const uint32_t words = sizeof(FrameArgs) / 4;
+  static_assert(sizeof(FrameArgs) % 4 == 0, "FrameArgs is copied word by word");
+  for (uint32_t i = threadIdx.x; i < count * words; i += blockDim.x)
+    reinterpret_cast<uint32_t*>(table + first)[i] = reinterpret_cast<const uint32_t*>(C.f)[i];
+}
+
 // TMD_VALIDATE, part 1 (before anything indexes with the counts): per-track fields and the two totals.
-__global__ void k_validate(DevGeo G, tmd_compressed in, const uint32_t* __restrict__ off, uint32_t* __restrict__ err) {
-  __shared__ unsigned long long s_sum;
-  if (threadIdx.x == 0) s_sum = 0;
+// The sum of trk_ncl is taken in 64 bits (the 32-bit offsets wrap for malformed counts).
+__global__ void k_validate(DevGeo G, tmd_compressed in, uint32_t* __restrict__ err) {
+  __shared__ unsigned long long s_sum, s_ncl;
+  if (threadIdx.x == 0) { s_sum = 0; s_ncl = 0; }
   __syncthreads();
   uint32_t bad = 0;
-  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < in.n_tracks; t += gridDim.x * blockDim.x)
-    bad |= (in.trk_ncl[t] < 1) | (in.trk_row0[t] >= G.n_rows) | (in.trk_sec0[t] >= G.n_az * G.n_sides);
+  unsigned long long ncl = 0;
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < in.n_tracks; t += gridDim.x * blockDim.x) {
+    const uint32_t n = in.trk_ncl[t];
+    ncl += n;
+    bad |= (n < 1) | (in.trk_row0[t] >= G.n_rows) | (in.trk_sec0[t] >= G.n_az * G.n_sides);
+  }
   if (bad) atomicOr(&err[ERR_TRACK_FIELD], 1u);
+  atomicAdd(&s_ncl, ncl);
   if (blockIdx.x == 0) {
     unsigned long long s = 0;
     for (uint32_t b = threadIdx.x; b < G.n_bins; b += blockDim.x) s += in.u_bin_count[b];
     atomicAdd(&s_sum, s);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      if (s_sum != in.n_unattached) atomicOr(&err[ERR_TRACK_FIELD], 2u);
-      if (in.n_tracks > 0 && off[in.n_tracks] != (uint32_t)in.n_attached) atomicOr(&err[ERR_TRACK_FIELD], 4u);
-    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    atomicAdd(reinterpret_cast<unsigned long long*>(err + ERR_NCL_SUM_LO), s_ncl);
+    if (blockIdx.x == 0 && s_sum != in.n_unattached) atomicOr(&err[ERR_TRACK_FIELD], 2u);
   }
 }
 
@@ -130,25 +148,174 @@ int check_args(const tmd_ctx* ctx, const tmd_compressed* in, const tmd_output* o
   return TMD_OK;
 }
 
-// Launch bookkeeping: TMD_BEFORE(stream) ... kernel<<<>>> ... TMD_AFTER(name, stream)
-#define TMD_BEFORE(stream)                                                                                  \
-  do {                                                                                                      \
-    if (timing && ctx->launches < TMD_MAX_KERNELS &&                                                        \
-        cudaEventRecord(ctx->ev_t0[ctx->launches], stream) != cudaSuccess) return TMD_ERR_CUDA;             \
-  } while (0)
-#define TMD_AFTER(name, stream)                                                                             \
-  do {                                                                                                      \
-    if (cudaGetLastError() != cudaSuccess) return TMD_ERR_CUDA;                                             \
-    if (timing && ctx->launches < TMD_MAX_KERNELS) {                                                        \
-      ctx->kernel_names[ctx->launches] = name;                                                              \
-      if (cudaEventRecord(ctx->ev_t1[ctx->launches], stream) != cudaSuccess) return TMD_ERR_CUDA;           \
-    }                                                                                                       \
-    ctx->launches++;                                                                                        \
-  } while (0)
+// argument / alignment / workspace checks of one frame and its FrameArgs
+int make_frame(const tmd_ctx* ctx, const tmd_compressed* in, const tmd_output* out, uint32_t flags, FrameArgs* F) {
+  int rc = check_args(ctx, in, out, true);
+  if (rc != TMD_OK) return rc;
+  const Workspace W = layout(ctx->geo.n_bins, in->n_tracks, in->n_attached, ctx->n_sm);
+  if (!out->workspace || out->workspace_bytes < W.total) return TMD_ERR_WORKSPACE;
+  if (misaligned(out->workspace, ALIGN)) return TMD_ERR_ALIGN;
+  F->in = *in;
+  F->clusters = (uint4*)out->clusters;
+  F->bin_offset = out->bin_offset;
+  F->probe_state = out->probe_state;
+  F->probe_step = out->probe_step;
+  F->validate = (flags & TMD_VALIDATE) ? 1u : 0u;
+  F->ws = (unsigned char*)out->workspace;
+  F->W = W;
+  return TMD_OK;
+}
+
 #define TMD_CUDA(call)                                   \
   do {                                                   \
     if ((call) != cudaSuccess) return TMD_ERR_CUDA;      \
   } while (0)
+
+// Launch bookkeeping: an event pair around the kernel with TMD_TIMING
+struct Launcher {
+  tmd_ctx* ctx;
+  cudaStream_t st;
+  bool timing;
+  int n = 0;
+  bool before() {
+    return !(timing && n < TMD_MAX_KERNELS && cudaEventRecord(ctx->ev_t0[n], st) != cudaSuccess);
+  }
+  bool after(const char* name) {
+    if (cudaGetLastError() != cudaSuccess) return false;
+    if (timing && n < TMD_MAX_KERNELS) {
+      ctx->kernel_names[n] = name;
+      if (cudaEventRecord(ctx->ev_t1[n], st) != cudaSuccess) return false;
+    }
+    ++n;
+    return true;
+  }
+};
+#define TMD_LAUNCH(name, ...)                      \
+  do {                                             \
+    if (!L.before()) return TMD_ERR_CUDA;          \
+    __VA_ARGS__;                                   \
+    if (!L.after(name)) return TMD_ERR_CUDA;       \
+  } while (0)
+
+// The launch sequence of rows A1-A7 over `n_frames` frames.  BATCH = false: one frame, its FrameArgs
+// passed by value.  BATCH = true: the frames' FrameArgs are in device memory (`table`) and every grid has a frame
+// coordinate; `mx` holds the per-kernel maxima of the frames' grid extents.
+struct Extents { uint32_t n_tiles, n_tracks, n_chunks, n_groups; bool any_probe; };
+
+template <bool BATCH>
+int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t n_frames, const Extents& mx, Launcher& L) {
+  const DevGeo& G = ctx->geo;
+  const uint32_t n_bins = G.n_bins, nf = n_frames;
+  cudaStream_t st = L.st;
+  const uint32_t bin_blocks = (n_bins + 255) / 256;
+  if (mx.n_tracks > 0) {
+    // A1: track offsets
+    TMD_LAUNCH("track_tile_sums", k_track_tile_sums<BATCH><<<dim3(mx.n_tiles, nf), SCAN_THREADS, 0, st>>>(F0, table));
+    TMD_LAUNCH("scan_tile_sums", k_scan_tile_sums<BATCH><<<dim3(1, nf), 1024, 0, st>>>(F0, table));
+    TMD_LAUNCH("track_offsets", k_track_offsets<BATCH><<<dim3(mx.n_tiles, nf), SCAN_THREADS, 0, st>>>(F0, table));
+    // A2: load-balance order (counting sort by cluster count, longest first, inside windows of consecutive tracks)
+    TMD_LAUNCH("len_sort_window",
+               k_len_sort_window<BATCH><<<dim3((mx.n_tracks + SORT_WINDOW - 1) / SORT_WINDOW, nf), SORT_THREADS, 0, st>>>(F0, table));
+    // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
+    const dim3 dg((mx.n_tracks + DECODE_THREADS - 1) / DECODE_THREADS, nf);
+    if (mx.any_probe) TMD_LAUNCH("track_decode", k_track_decode<true, BATCH><<<dg, DECODE_THREADS, ctx->decode_smem, st>>>(G, F0, table));
+    else TMD_LAUNCH("track_decode", k_track_decode<false, BATCH><<<dg, DECODE_THREADS, ctx->decode_smem, st>>>(G, F0, table));
+    // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
+    uint32_t per_sm = (uint32_t)(ctx->smem_per_sm / (ctx->rank_smem + 1024));
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 16) per_sm = 16;
+    uint32_t rank_blocks = (mx.n_chunks + WR_WARPS - 1) / WR_WARPS;
+    const uint32_t rank_cap = (per_sm * (uint32_t)ctx->n_sm + nf - 1) / nf;
+    if (rank_blocks > rank_cap) rank_blocks = rank_cap;
+    if (rank_blocks < 1) rank_blocks = 1;
+    TMD_LAUNCH("rank", k_rank<BATCH><<<dim3(rank_blocks, nf), WR_THREADS, ctx->rank_smem, st>>>(G, F0, table));
+    // A4: column scan over chunks
+    TMD_LAUNCH("col_group_sums", k_col_group_sums<BATCH><<<dim3(bin_blocks, mx.n_groups, nf), 256, 0, st>>>(n_bins, F0, table));
+  }
+  // att_cnt (zero for a frame without tracks), then bin offsets
+  TMD_LAUNCH("col_group_scan", k_col_group_scan<BATCH><<<dim3(bin_blocks, nf), 256, 0, st>>>(n_bins, F0, table));
+  TMD_LAUNCH("bin_offsets", k_bin_offsets<BATCH><<<dim3(1, nf), 1024, 0, st>>>(n_bins, F0, table));
+  if (mx.n_tracks > 0)
+    TMD_LAUNCH("col_apply", k_col_apply<BATCH><<<dim3(bin_blocks, mx.n_groups, nf), 256, 0, st>>>(n_bins, F0, table));
+  // A7: unattached clusters
+  TMD_LAUNCH("unattached", k_unattached<BATCH><<<dim3(n_bins, nf), UNATT_THREADS, 0, st>>>(G, F0, table));
+  if (mx.n_tracks > 0) {
+    // A6: copy-through + scatter (a thread-block cluster of SC_CLUSTER CTAs per chunk)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(mx.n_chunks * SC_CLUSTER, nf);
+    cfg.blockDim = dim3(SC_THREADS);
+    cfg.dynamicSmemBytes = ctx->scatter_smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = SC_CLUSTER; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    TMD_LAUNCH("scatter", if (cudaLaunchKernelEx(&cfg, k_scatter<BATCH>, G, F0, table) != cudaSuccess) return TMD_ERR_CUDA);
+  }
+  return TMD_OK;
+}
+
+int prepare_timing(tmd_ctx* ctx, bool timing) {
+  ctx->timing_valid = false;
+  if (timing && !ctx->events_created) {
+    for (int i = 0; i < TMD_MAX_KERNELS; ++i) {
+      TMD_CUDA(cudaEventCreate(&ctx->ev_t0[i]));
+      TMD_CUDA(cudaEventCreate(&ctx->ev_t1[i]));
+    }
+    ctx->events_created = true;
+  }
+  return TMD_OK;
+}
+
+// tmd_selftest_ieee: the unchecked IEEE sequences of the decode kernel against the intrinsics they replace.
+// counts[0]: sqrt_rn_safe vs __fsqrt_rn on EVERY binary32 pattern in [2^-100, 2^100];
+// counts[1]: div_rn_safe vs __fdiv_rn on 2^log2_pairs hashed (dividend, divisor) pairs, |dividend| in [2^-40, 2^84],
+//            |divisor| in [2^-10, 2^80], plus every combination of 16 edge mantissas and all exponents of those ranges;
+// counts[2]: floor_clamp vs (int)clamp(floorf(w), 0, hi) on every binary32 pattern, both limits.
+__device__ __forceinline__ uint32_t mix32(uint32_t x) {
+  x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+  return x;
+}
+__device__ __forceinline__ bool same_float(float a, float b) {
+  return __float_as_uint(a) == __float_as_uint(b) || (a != a && b != b);
+}
+__device__ __forceinline__ bool div_agrees(float a, float b) { return same_float(div_rn_safe(a, b, recip_refined(b)), __fdiv_rn(a, b)); }
+
+__global__ void k_selftest_ieee(uint32_t log2_pairs, unsigned long long* __restrict__ counts) {
+  const uint64_t tid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, nthr = (uint64_t)gridDim.x * blockDim.x;
+  unsigned long long bad_sqrt = 0, bad_div = 0, bad_floor = 0;
+  for (uint64_t v = tid; v < (1ull << 32); v += nthr) {
+    const float x = __uint_as_float((uint32_t)v);
+    if (x >= 7.888609052210118e-31f && x <= 1.2676506002282294e30f) bad_sqrt += !same_float(sqrt_rn_safe(x), __fsqrt_rn(x));
+    const uint32_t wantP = (uint32_t)(int)clampf(floorf(x), 0.0f, 65535.0f), wantT = (uint32_t)(int)clampf(floorf(x), 0.0f, 16777215.0f);
+    bad_floor += (floor_clamp(x, 65535) != wantP) + (floor_clamp(x, 16777215) != wantT);
+  }
+  const uint64_t n_pairs = 1ull << log2_pairs;
+  for (uint64_t v = tid; v < n_pairs; v += nthr) {
+    const uint32_t h1 = mix32((uint32_t)v * 2u + 1u), h2 = mix32(h1 ^ (uint32_t)(v >> 31) ^ 0x9e3779b9u), h3 = mix32(h2 + 0x85ebca6bu);
+    const uint32_t ea = 127u - 40u + h3 % 125u;            // dividend exponent 2^-40 .. 2^84
+    const uint32_t eb = 127u - 10u + (h3 >> 8) % 91u;      // divisor exponent 2^-10 .. 2^80
+    const float a = __uint_as_float((h1 & 0x807FFFFFu) | (ea << 23)), b = __uint_as_float((h2 & 0x807FFFFFu) | (eb << 23));
+    bad_div += !div_agrees(a, b);
+  }
+  const uint32_t edge[16] = {0u, 1u, 2u, 0x7FFFFFu, 0x7FFFFEu, 0x400000u, 0x400001u, 0x3FFFFFu, 0x555555u, 0x2AAAAAu, 0x000FFFu, 0x7FF000u,
+                             0x100000u, 0x600000u, 0x123456u, 0x654321u};
+  for (uint64_t v = tid; v < 125ull * 91ull * 256ull * 4ull; v += nthr) {
+    const uint32_t ia = (uint32_t)(v % 125), ib = (uint32_t)(v / 125 % 91), m = (uint32_t)(v / (125 * 91) % 256), sg = (uint32_t)(v / (125 * 91 * 256));
+    const float a = __uint_as_float(edge[m & 15] | ((127u - 40u + ia) << 23) | ((sg & 1u) << 31));
+    const float b = __uint_as_float(edge[m >> 4] | ((127u - 10u + ib) << 23) | ((sg >> 1) << 31));
+    bad_div += !div_agrees(a, b);
+  }
+  if (bad_sqrt) atomicAdd(&counts[0], bad_sqrt);
+  if (bad_div) atomicAdd(&counts[1], bad_div);
+  if (bad_floor) atomicAdd(&counts[2], bad_floor);
+}
+
+template <typename K>
+cudaError_t allow_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
 
 }  // namespace
 
@@ -160,6 +327,13 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   if (g->n_az < 1 || g->n_az > 63 || g->n_sides < 1 || g->n_sides > 2 || g->n_rows < 1 || g->n_rows > 255) return TMD_ERR_ARG;
   if (g->n_sectors_out < 1 || g->n_sectors_out > g->n_az * g->n_sides) return TMD_ERR_ARG;
   if ((uint64_t)g->n_sectors_out * g->n_rows > MAX_BINS) return TMD_ERR_ARG;
+  // finite, bounded tables (bounds: tmd_decode.cuh TMD_GEO_*): they keep every magnitude of the model far from overflow
+  if (!(fabsf(f->bz_tesla) <= TMD_MAX_BZ) || !(fabsf(g->cos_a) <= 1.0f) || !(fabsf(g->sin_a) <= 1.0f)) return TMD_ERR_ARG;
+  for (uint32_t r = 0; r < g->n_rows; ++r) {
+    if (!(fabsf(g->row_x[r]) <= TMD_GEO_MAX_X) || !(g->row_padw[r] >= TMD_GEO_MIN_PADW && g->row_padw[r] <= TMD_GEO_MAX_PADW) ||
+        !(g->row_inv_padw[r] >= 1.0f / TMD_GEO_MAX_PADW && g->row_inv_padw[r] <= 1.0f / TMD_GEO_MIN_PADW))
+      return TMD_ERR_ARG;
+  }
   tmd_ctx* ctx = new (std::nothrow) tmd_ctx();
   if (!ctx) return TMD_ERR_CUDA;
   memset(ctx, 0, sizeof(*ctx));
@@ -175,29 +349,49 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   cudaError_t e = cudaMalloc(&ctx->d_rows, sizeof(RowGeo) * g->n_rows);
   if (e == cudaSuccess) e = cudaMemcpy(ctx->d_rows, h, sizeof(RowGeo) * g->n_rows, cudaMemcpyHostToDevice);
   free(h);
+  int smem_sm = 0;
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, ctx->device);
+  ctx->smem_per_sm = (size_t)smem_sm;
   const uint32_t n_bins_c = g->n_sectors_out * g->n_rows;
   ctx->rank_smem = (size_t)WR_WARPS * wr_warp_smem(n_bins_c);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->rank_smem);
   ctx->scatter_smem = sc_smem_bytes(n_bins_c);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->scatter_smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scatter, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
   ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_track_decode<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(k_track_decode<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->decode_smem);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
-  if (e == cudaSuccess) {
-    int lo = 0, hi = 0;   // numerically lowest = highest priority: the short integer kernels should not queue behind the decode
-    e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
-    if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&ctx->side, cudaStreamNonBlocking, hi);
-  }
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
+  // The dynamic shared-memory limit is a per-function, process-wide attribute: always set it to the maximum any geometry
+  // can need (MAX_BINS bins, 255 rows), so that contexts of different geometries never lower it for one another.
+  const size_t rank_max = (size_t)WR_WARPS * wr_warp_smem(MAX_BINS), scatter_max = sc_smem_bytes(MAX_BINS);
+  const size_t decode_max = DECODE_STAGE_BYTES + sizeof(RowGeo) * 255;
+  if (e == cudaSuccess) e = allow_smem(k_rank<false>, rank_max);
+  if (e == cudaSuccess) e = allow_smem(k_rank<true>, rank_max);
+  if (e == cudaSuccess) e = allow_smem(k_scatter<false>, scatter_max);
+  if (e == cudaSuccess) e = allow_smem(k_scatter<true>, scatter_max);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scatter<false>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scatter<true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  if (e == cudaSuccess) e = allow_smem(k_track_decode<false, false>, decode_max);
+  if (e == cudaSuccess) e = allow_smem(k_track_decode<true, false>, decode_max);
+  if (e == cudaSuccess) e = allow_smem(k_track_decode<false, true>, decode_max);
+  if (e == cudaSuccess) e = allow_smem(k_track_decode<true, true>, decode_max);
   if (e != cudaSuccess) {
     cudaGetLastError();
     tmd_destroy(ctx);
     return TMD_ERR_CUDA;
+  }
+  {  // the scatter kernel needs a thread-block cluster of SC_CLUSTER CTAs: say so here, not at the first decode
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(SC_CLUSTER);
+    cfg.blockDim = dim3(SC_THREADS);
+    cfg.dynamicSmemBytes = ctx->scatter_smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = SC_CLUSTER; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n_clusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&n_clusters, k_scatter<false>, &cfg) != cudaSuccess || n_clusters < 1) {
+      cudaGetLastError();
+      tmd_destroy(ctx);
+      return TMD_ERR_DEVICE;
+    }
   }
   DevGeo& G = ctx->geo;
   G.n_az = g->n_az; G.n_sides = g->n_sides; G.n_sectors_out = g->n_sectors_out; G.n_rows = g->n_rows;
@@ -217,153 +411,39 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
 int tmd_workspace_bytes(const tmd_ctx* ctx, uint32_t n_tracks, uint64_t n_att, uint64_t n_unatt, size_t* out_bytes) {
   if (!ctx || !out_bytes) return TMD_ERR_ARG;
   if (n_att + n_unatt > TMD_MAX_CLUSTERS || n_att < n_tracks) return TMD_ERR_ARG;
-  *out_bytes = layout(ctx->geo.n_bins, n_tracks, n_att).total;
+  *out_bytes = layout(ctx->geo.n_bins, n_tracks, n_att, ctx->n_sm).total;
   return TMD_OK;
 }
 
 int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
-  int rc = check_args(ctx, in, out, true);
+  FrameArgs F;
+  int rc = make_frame(ctx, in, out, flags, &F);
   if (rc != TMD_OK) return rc;
-  const DevGeo& G = ctx->geo;
-  const uint32_t n_trk = in->n_tracks, n_bins = G.n_bins;
-  const uint32_t n_att = (uint32_t)in->n_attached, n_un = (uint32_t)in->n_unattached;
-  const Workspace W = layout(n_bins, n_trk, n_att);
-  if (!out->workspace || out->workspace_bytes < W.total) return TMD_ERR_WORKSPACE;
-  if (misaligned(out->workspace, ALIGN)) return TMD_ERR_ALIGN;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  unsigned char* ws = (unsigned char*)out->workspace;
-  uint32_t* d_err = (uint32_t*)(ws + W.o_err);
-  uint32_t* d_tile = (uint32_t*)(ws + W.o_tile_sum);
-  uint32_t* d_off = (uint32_t*)(ws + W.o_off);
-  uint32_t* d_perm = (uint32_t*)(ws + W.o_perm);
-  uint32_t* d_attcnt = (uint32_t*)(ws + W.o_att_cnt);
-  uint32_t* d_ustart = (uint32_t*)(ws + W.o_u_start);
-  uint32_t* d_gsum = (uint32_t*)(ws + W.o_gsum);
-  uint16_t* d_hist = (uint16_t*)(ws + W.o_hist);
-  uint16_t* d_start16 = (uint16_t*)(ws + W.o_start16);
-  uint32_t* d_rel = (uint32_t*)(ws + W.o_rel);
-  uint16_t* d_rank = (uint16_t*)(ws + W.o_rank16);
-  uint2* d_inter = (uint2*)(ws + W.o_inter);
   const bool validate = (flags & TMD_VALIDATE) != 0, timing = (flags & TMD_TIMING) != 0;
-  cudaStream_t s2 = (flags & TMD_SERIAL) ? st : ctx->side;   // TMD_SERIAL: one stream, kernels back to back
-  ctx->launches = 0;
-  ctx->timing_valid = false;
-  if (timing && !ctx->events_created) {
-    for (int i = 0; i < TMD_MAX_KERNELS; ++i) {
-      TMD_CUDA(cudaEventCreate(&ctx->ev_t0[i]));
-      TMD_CUDA(cudaEventCreate(&ctx->ev_t1[i]));
-    }
-    ctx->events_created = true;
-  }
-  TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
-
-  if (n_trk > 0) {  // A1: track offsets
-    TMD_BEFORE(st);
-    k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile);
-    TMD_AFTER("track_tile_sums", st);
-    TMD_BEFORE(st);
-    k_scan_tile_sums<<<1, 1024, 0, st>>>(d_tile, W.n_tiles);
-    TMD_AFTER("scan_tile_sums", st);
-    TMD_BEFORE(st);
-    k_track_offsets<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_tile, W.n_tiles, d_off);
-    TMD_AFTER("track_offsets", st);
-  }
+  rc = prepare_timing(ctx, timing);
+  if (rc != TMD_OK) return rc;
+  uint32_t* d_err = F.at<uint32_t>(F.W.o_err);
   if (validate) {
-    TMD_BEFORE(st);
-    k_validate<<<ctx->n_sm, 256, 0, st>>>(G, *in, d_off, d_err);
-    TMD_AFTER("validate", st);
+    // part 1, before anything indexes with the counts: per-track fields, sum(trk_ncl) in 64 bits, sum(u_bin_count)
     uint32_t h_err[ERR_WORDS];
+    TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
+    k_validate<<<ctx->n_sm, 256, 0, st>>>(ctx->geo, *in, d_err);
+    TMD_CUDA(cudaGetLastError());
     TMD_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
     TMD_CUDA(cudaStreamSynchronize(st));
-    if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;
+    const uint64_t ncl_sum = (uint64_t)h_err[ERR_NCL_SUM_LO] | ((uint64_t)h_err[ERR_NCL_SUM_HI] << 32);
+    if (h_err[ERR_TRACK_FIELD] || ncl_sum != in->n_attached) return TMD_ERR_CORRUPT;
+    TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
   }
-  if (n_trk > 0) {
-    // A2: load-balance order (counting sort by cluster count, longest first, inside windows of consecutive tracks)
-    TMD_BEFORE(st);
-    k_len_sort_window<<<(n_trk + SORT_WINDOW - 1) / SORT_WINDOW, SORT_THREADS, 0, st>>>(in->trk_ncl, n_trk, d_perm);
-    TMD_AFTER("len_sort_window", st);
-    // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
-    DecodeArgs D;
-    D.off = d_off; D.perm = d_perm; D.in = *in; D.inter = d_inter;
-    D.probe_state = out->probe_state; D.probe_step = out->probe_step; D.err = d_err;
-    TMD_BEFORE(st);
-    const uint32_t decode_blocks = (n_trk + DECODE_THREADS - 1) / DECODE_THREADS;
-    if (out->probe_state) k_track_decode<true><<<decode_blocks, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
-    else k_track_decode<false><<<decode_blocks, DECODE_THREADS, ctx->decode_smem, st>>>(G, D);
-    TMD_AFTER("track_decode", st);
-    // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
-    RankArgs R;
-    R.inter = d_inter; R.hist = d_hist; R.rank16 = d_rank; R.n_attached = n_att; R.n_chunks = W.n_chunks; R.chunk_shift = W.chunk_shift; R.start16 = d_start16; R.start_stride = sc_start_stride(n_bins);
-    uint32_t per_sm = (uint32_t)((size_t)(227 * 1024) / (ctx->rank_smem + 1024));
-    if (per_sm < 1) per_sm = 1;
-    if (per_sm > 16) per_sm = 16;
-    uint32_t rank_blocks = (W.n_chunks + WR_WARPS - 1) / WR_WARPS;
-    if (rank_blocks > per_sm * (uint32_t)ctx->n_sm) rank_blocks = per_sm * (uint32_t)ctx->n_sm;
-    TMD_BEFORE(st);
-    k_rank<<<rank_blocks, WR_THREADS, ctx->rank_smem, st>>>(G, R);
-    TMD_AFTER("rank", st);
-    // A4: column scan over chunks
-    dim3 cg((n_bins + 255) / 256, W.n_groups);
-    TMD_BEFORE(st);
-    k_col_group_sums<<<cg, 256, 0, st>>>(d_hist, W.n_chunks, n_bins, d_gsum);
-    TMD_AFTER("col_group_sums", st);
-    TMD_BEFORE(st);
-    k_col_group_scan<<<(n_bins + 255) / 256, 256, 0, st>>>(d_gsum, W.n_groups, n_bins, d_attcnt);
-    TMD_AFTER("col_group_scan", st);
-  } else {
-    TMD_CUDA(cudaMemsetAsync(d_attcnt, 0, (size_t)n_bins * 4, st));
-  }
-  TMD_BEFORE(st);
-  k_bin_offsets<<<1, 1024, 0, st>>>(d_attcnt, in->u_bin_count, n_bins, out->bin_offset, d_ustart);
-  TMD_AFTER("bin_offsets", st);
-  if (n_trk > 0) {
-    dim3 cg((n_bins + 255) / 256, W.n_groups);
-    TMD_BEFORE(st);
-    k_col_apply<<<cg, 256, 0, st>>>(d_hist, d_gsum, out->bin_offset, W.n_chunks, n_bins, d_rel);
-    TMD_AFTER("col_apply", st);
-  }
-  // ---- fork: A7 (unattached clusters) on the context's second stream, next to A6 on the caller's
-  const bool fork = n_un > 0 && n_trk > 0 && s2 != st;
-  if (n_un > 0) {
-    cudaStream_t su = fork ? s2 : st;
-    if (fork) {
-      TMD_CUDA(cudaEventRecord(ctx->ev_fork, st));
-      TMD_CUDA(cudaStreamWaitEvent(s2, ctx->ev_fork, 0));
-    }
-    UnattachedArgs U;
-    U.in = *in; U.u_start = d_ustart; U.bin_offset = out->bin_offset; U.att_cnt = d_attcnt;
-    U.clusters = (uint4*)out->clusters; U.n_clusters_total = n_att + n_un;
-    TMD_BEFORE(su);
-    k_unattached<<<n_bins, UNATT_THREADS, 0, su>>>(G, U);
-    TMD_AFTER("unattached", su);
-    if (fork) TMD_CUDA(cudaEventRecord(ctx->ev_join, s2));
-  }
-  if (n_trk > 0) {
-    // A6: copy-through + scatter
-    ScatterArgs S;
-    S.inter = d_inter; S.rank16 = d_rank; S.rel = d_rel;
-    S.a_qtot = in->a_qtot; S.a_qmax = in->a_qmax; S.a_flags = in->a_flags; S.a_sigpad = in->a_sigpad; S.a_sigtime = in->a_sigtime;
-    S.clusters = (uint4*)out->clusters; S.n_attached = n_att; S.n_clusters_total = n_att + n_un; S.chunk_shift = W.chunk_shift;
-    S.start16 = d_start16; S.start_stride = sc_start_stride(n_bins);
-    TMD_BEFORE(st);
-    {
-      cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3(W.n_chunks * SC_CLUSTER);
-      cfg.blockDim = dim3(SC_THREADS);
-      cfg.dynamicSmemBytes = ctx->scatter_smem;
-      cfg.stream = st;
-      cudaLaunchAttribute attr[1];
-      attr[0].id = cudaLaunchAttributeClusterDimension;
-      attr[0].val.clusterDim.x = SC_CLUSTER; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-      cfg.attrs = attr;
-      cfg.numAttrs = 1;
-      if (cudaLaunchKernelEx(&cfg, k_scatter, G, S) != cudaSuccess) return TMD_ERR_CUDA;
-    }
-    TMD_AFTER("scatter", st);
-  }
-  if (fork) TMD_CUDA(cudaStreamWaitEvent(st, ctx->ev_join, 0));   // join: everything is ordered before later work on `st`
+  Launcher L{ctx, st, timing};
+  const Extents mx = {F.W.n_tiles, in->n_tracks, F.W.n_chunks, F.W.n_groups, out->probe_state != nullptr};
+  rc = enqueue<false>(ctx, F, nullptr, 1, mx, L);
+  ctx->launches = L.n + (validate ? 1 : 0);
+  if (rc != TMD_OK) return rc;
+  ctx->timed_launches = L.n;
   ctx->timing_valid = timing;
-  if (validate) {
+  if (validate) {   // part 2: a decoded sector without output bins (reading 20)
     uint32_t h_err[ERR_WORDS];
     TMD_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
     TMD_CUDA(cudaStreamSynchronize(st));
@@ -372,10 +452,62 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
   return TMD_OK;
 }
 
+int tmd_decode_batch(tmd_ctx* ctx, uint32_t n_frames, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
+  if (!ctx || !in || !out || n_frames < 1 || n_frames > TMD_MAX_BATCH) return TMD_ERR_ARG;
+  if (flags & TMD_VALIDATE) return TMD_ERR_ARG;          // it synchronises: validate frames one by one with tmd_decode
+  if (n_frames == 1) return tmd_decode(ctx, in, out, flags, cuda_stream);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool timing = (flags & TMD_TIMING) != 0;
+  int rc = prepare_timing(ctx, timing);
+  if (rc != TMD_OK) return rc;
+  Extents mx = {0, 0, 0, 0, false};
+  FrameArgs* table = nullptr;
+  FrameChunk chunk;
+  // Chunk size of the batch: the one a single frame holding ALL the attached clusters would get (larger than any
+  // frame's own, so its tables fit the frame's workspace): a batch has chunks enough with every frame cut coarsely.
+  uint64_t att_total = 0;
+  for (uint32_t i = 0; i < n_frames; ++i) att_total += in[i].n_attached;
+  const uint32_t batch_shift = layout(ctx->geo.n_bins, 0, att_total, ctx->n_sm).chunk_shift;
+  auto make_batch_frame = [&](uint32_t i, FrameArgs* F) -> int {
+    const int r = make_frame(ctx, &in[i], &out[i], flags, F);
+    if (r != TMD_OK) return r;
+    if (batch_shift > F->W.chunk_shift) {
+      F->W.chunk_shift = batch_shift;
+      F->W.n_chunks = (uint32_t)((in[i].n_attached + (1ull << batch_shift) - 1) >> batch_shift);
+      F->W.n_groups = (F->W.n_chunks + COL_GROUP - 1) / COL_GROUP;
+    }
+    return TMD_OK;
+  };
+  // every frame is checked before anything is enqueued
+  for (uint32_t i = 0; i < n_frames; ++i) {
+    FrameArgs F;
+    rc = make_batch_frame(i, &F);
+    if (rc != TMD_OK) return rc;
+    if (i == 0) table = F.at<FrameArgs>(F.W.o_table);
+    mx.n_tiles = mx.n_tiles > F.W.n_tiles ? mx.n_tiles : F.W.n_tiles;
+    mx.n_tracks = mx.n_tracks > in[i].n_tracks ? mx.n_tracks : in[i].n_tracks;
+    mx.n_chunks = mx.n_chunks > F.W.n_chunks ? mx.n_chunks : F.W.n_chunks;
+    mx.n_groups = mx.n_groups > F.W.n_groups ? mx.n_groups : F.W.n_groups;
+    mx.any_probe = mx.any_probe || out[i].probe_state != nullptr;
+  }
+  Launcher L{ctx, st, timing};
+  for (uint32_t first = 0; first < n_frames; first += STORE_FRAMES) {
+    const uint32_t count = n_frames - first < STORE_FRAMES ? n_frames - first : STORE_FRAMES;
+    for (uint32_t k = 0; k < count; ++k) make_batch_frame(first + k, &chunk.f[k]);
+    TMD_LAUNCH("store_frames", k_store_frames<<<1, 256, 0, st>>>(chunk, table, first, count));
+  }
+  rc = enqueue<true>(ctx, chunk.f[0], table, n_frames, mx, L);
+  ctx->launches = L.n;
+  if (rc != TMD_OK) return rc;
+  ctx->timed_launches = L.n;
+  ctx->timing_valid = timing;
+  return TMD_OK;
+}
+
 int tmd_kernel_times(tmd_ctx* ctx, int max_kernels, const char** names, float* ms) {
   if (!ctx || !names || !ms || max_kernels < 0) return TMD_ERR_ARG;
   if (!ctx->timing_valid) return 0;
-  const int n = ctx->launches < TMD_MAX_KERNELS ? ctx->launches : TMD_MAX_KERNELS;
+  const int n = ctx->timed_launches < TMD_MAX_KERNELS ? ctx->timed_launches : TMD_MAX_KERNELS;
   int k = 0;
   for (; k < n && k < max_kernels; ++k) {
     names[k] = ctx->kernel_names[k];
@@ -396,18 +528,21 @@ int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compress
   for (void* p : outs) if (!p) return TMD_ERR_ARG;
   if (in->n_attached > in->n_tracks && (!out->a_rowdiff || !out->a_secleg || !out->a_padres || !out->a_timeres)) return TMD_ERR_ARG;
   if (misaligned(in->trk_ncl, 16) || misaligned(in->att, 16)) return TMD_ERR_ALIGN;
-  const Workspace W = layout(ctx->geo.n_bins, in->n_tracks, in->n_attached);
+  const Workspace W = layout(ctx->geo.n_bins, in->n_tracks, in->n_attached, ctx->n_sm);
   if (!workspace || workspace_bytes < W.total) return TMD_ERR_WORKSPACE;
   if (misaligned(workspace, ALIGN)) return TMD_ERR_ALIGN;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  unsigned char* ws = (unsigned char*)workspace;
-  uint32_t* d_err = (uint32_t*)(ws + W.o_err);
-  uint32_t* d_tile = (uint32_t*)(ws + W.o_tile_sum);
-  uint32_t* d_off = (uint32_t*)(ws + W.o_off);
+  FrameArgs F;
+  memset(&F, 0, sizeof(F));
+  F.in.n_tracks = in->n_tracks; F.in.n_attached = in->n_attached; F.in.trk_ncl = in->trk_ncl;
+  F.ws = (unsigned char*)workspace;
+  F.W = W;
+  uint32_t* d_err = F.at<uint32_t>(W.o_err);
+  uint32_t* d_off = F.at<uint32_t>(W.o_off);
   if (cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st) != cudaSuccess) return TMD_ERR_CUDA;
-  k_track_tile_sums<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, in->n_tracks, d_tile);
-  k_scan_tile_sums<<<1, 1024, 0, st>>>(d_tile, W.n_tiles);
-  k_track_offsets<<<W.n_tiles, SCAN_THREADS, 0, st>>>(in->trk_ncl, in->n_tracks, d_tile, W.n_tiles, d_off);
+  k_track_tile_sums<false><<<W.n_tiles, SCAN_THREADS, 0, st>>>(F, nullptr);
+  k_scan_tile_sums<false><<<1, 1024, 0, st>>>(F, nullptr);
+  k_track_offsets<false><<<W.n_tiles, SCAN_THREADS, 0, st>>>(F, nullptr);
   EncodeArgs E;
   E.n_tracks = in->n_tracks; E.off = d_off; E.trk_qptf = in->trk_qptf; E.att = (const uint4*)in->att; E.leg = in->leg;
   E.trk_qpt = (int8_t*)out->trk_qpt; E.trk_row0 = (uint8_t*)out->trk_row0; E.trk_sec0 = (uint8_t*)out->trk_sec0;
@@ -441,7 +576,7 @@ static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out,
   }
   const uint32_t n_bins = ctx->geo.n_bins;
   const size_t n_trk = in->n_tracks, n_att = in->n_attached, n_res = n_att - n_trk, n_un = in->n_unattached;
-  const Workspace W = layout(n_bins, in->n_tracks, n_att);
+  const Workspace W = layout(n_bins, in->n_tracks, n_att, ctx->n_sm);
   // arena: inputs, outputs, workspace
   struct Seg { const void* src; size_t bytes; size_t at; };
   Seg segs[] = {
@@ -533,11 +668,28 @@ int tmd_host_wait(tmd_ctx* ctx, int slot) {
   return TMD_OK;
 }
 
+int tmd_selftest_ieee(uint32_t log2_pairs, uint64_t mismatches[3]) {
+  if (!mismatches || log2_pairs > 40) return TMD_ERR_ARG;
+  unsigned long long* d = nullptr;
+  int n_sm = 0, dev = 0;
+  TMD_CUDA(cudaGetDevice(&dev));
+  TMD_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  TMD_CUDA(cudaMalloc(&d, 3 * sizeof(unsigned long long)));
+  cudaError_t e = cudaMemset(d, 0, 3 * sizeof(unsigned long long));
+  if (e == cudaSuccess) {
+    k_selftest_ieee<<<n_sm * 8, 256>>>(log2_pairs, d);
+    e = cudaGetLastError();
+  }
+  unsigned long long h[3] = {0, 0, 0};
+  if (e == cudaSuccess) e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return TMD_ERR_CUDA;
+  for (int i = 0; i < 3; ++i) mismatches[i] = h[i];
+  return TMD_OK;
+}
+
 int tmd_destroy(tmd_ctx* ctx) {
   if (!ctx) return TMD_OK;
-  if (ctx->side) { cudaStreamSynchronize(ctx->side); cudaStreamDestroy(ctx->side); }
-  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   for (tmd_ctx::HostSlot& S : ctx->slots) {
     if (S.busy) cudaEventSynchronize(S.d2h_done);
     if (S.arena) cudaFree(S.arena);
@@ -559,6 +711,7 @@ const char* tmd_status_string(int status) {
     case TMD_ERR_WORKSPACE: return "workspace missing or too small";
     case TMD_ERR_CUDA: return "CUDA runtime error";
     case TMD_ERR_CORRUPT: return "inconsistent compressed input";
+    case TMD_ERR_DEVICE: return "device cannot run the kernels (thread-block clusters of 16 CTAs)";
     default: return "unknown status";
   }
 }

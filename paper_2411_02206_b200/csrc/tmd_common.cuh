@@ -34,8 +34,39 @@ struct DevGeo {
   const RowGeo* rows;   // DEVICE [n_rows]
 };
 
-// error word indices in the workspace (TMD_VALIDATE)
-enum { ERR_TRACK_FIELD = 0, ERR_SECTOR_OUT = 1, ERR_WORDS = 4 };
+// error words in the workspace (TMD_VALIDATE); words 2-3 hold the 64-bit sum of trk_ncl
+enum { ERR_TRACK_FIELD = 0, ERR_SECTOR_OUT = 1, ERR_NCL_SUM_LO = 2, ERR_NCL_SUM_HI = 3, ERR_WORDS = 4 };
+
+// Layout of one frame's workspace (byte offsets from its 256-byte aligned base) and the sizes derived from the frame's
+// counts.  A pure function of (n_bins, n_tracks, n_attached, SM count): tmd_workspace_bytes and tmd_decode agree.
+struct Workspace {
+  uint32_t n_tiles, n_chunks, n_groups, chunk_shift;
+  size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_start16, o_rel, o_rank16, o_inter, o_table, total;
+};
+
+// Everything the kernels need to know about ONE time frame.  tmd_decode passes it by value (kernel parameter space);
+// tmd_decode_batch keeps one per frame in device memory (frame 0's workspace) and the kernels pick theirs with the
+// frame coordinate of the grid, so that many small frames share one launch sequence.
+struct FrameArgs {
+  tmd_compressed in;         // DEVICE pointers
+  uint4* clusters;
+  uint32_t* bin_offset;
+  uint32_t* probe_state;     // nullable
+  uint32_t probe_step;
+  uint32_t validate;         // TMD_VALIDATE: report malformed fields in the error words
+  unsigned char* ws;         // this frame's workspace
+  Workspace W;
+
+  template <typename T>
+  __host__ __device__ __forceinline__ T* at(size_t offset) const { return reinterpret_cast<T*>(ws + offset); }
+  __host__ __device__ __forceinline__ uint32_t n_res() const { return (uint32_t)in.n_attached - in.n_tracks; }
+};
+
+// The frame a block works on: the by-value parameter, or entry `f` of the batch table.
+template <bool BATCH>
+__device__ __forceinline__ const FrameArgs& frame_of(const FrameArgs& F0, const FrameArgs* __restrict__ table, uint32_t f) {
+  return BATCH ? table[f] : F0;
+}
 
 // ---- the integer part of one step: leg / row / sector bookkeeping (C3-3, C3-4, C3-5 without the rotation) ----------
 struct WalkState {

@@ -30,6 +30,18 @@ struct RankArgs {
   uint32_t n_attached, n_chunks, chunk_shift, start_stride;
 };
 
+// row stride (entries) of the start16 table: n_bins + 1 entries, padded to 16 bytes
+__host__ __device__ inline uint32_t sc_start_stride(uint32_t n_bins) { return (n_bins + 1 + 7) & ~7u; }
+
+__device__ __forceinline__ RankArgs rank_args(const FrameArgs& F, uint32_t n_bins) {
+  RankArgs A;
+  A.inter = F.at<uint2>(F.W.o_inter); A.hist = F.at<uint16_t>(F.W.o_hist); A.rank16 = F.at<uint16_t>(F.W.o_rank16);
+  A.start16 = F.at<uint16_t>(F.W.o_start16);
+  A.n_attached = (uint32_t)F.in.n_attached; A.n_chunks = F.W.n_chunks; A.chunk_shift = F.W.chunk_shift;
+  A.start_stride = sc_start_stride(n_bins);
+  return A;
+}
+
 // bytes of dynamic shared memory per warp: cnt u16[n_bins], padded to 16 bytes
 __host__ __device__ inline uint32_t wr_warp_smem(uint32_t n_bins) { return (n_bins * 2 + 15) & ~15u; }
 
@@ -69,9 +81,12 @@ __device__ __forceinline__ uint32_t warp_rank32(uint16_t* cnt, uint32_t b, uint3
   return rank;
 }
 
-__global__ void __launch_bounds__(WR_THREADS) k_rank(DevGeo G, RankArgs A) {
+template <bool BATCH>
+__global__ void __launch_bounds__(WR_THREADS) k_rank(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
+                                                     const FrameArgs* __restrict__ table) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t lane = lane_id(), wib = threadIdx.x >> 5, n_bins = G.n_bins;
+  const RankArgs A = rank_args(frame_of<BATCH>(F0, table, blockIdx.y), n_bins);
   const uint32_t cnt_bytes = wr_warp_smem(n_bins);
   uint16_t* cnt = reinterpret_cast<uint16_t*>(smem_raw + (size_t)wib * cnt_bytes);
   const uint32_t n_warps = gridDim.x * WR_WARPS;

@@ -39,9 +39,14 @@ constexpr int SCAN_THREADS = 512;
 constexpr int SCAN_ITEMS = 8;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_track_tile_sums(const uint16_t* __restrict__ trk_ncl, uint32_t n_tracks,
-                                                                 uint32_t* __restrict__ tile_sum) {
+template <bool BATCH>
+__global__ void __launch_bounds__(SCAN_THREADS) k_track_tile_sums(const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
   __shared__ uint32_t ws[33];
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
+  if (blockIdx.x >= F.W.n_tiles) return;
+  const uint16_t* __restrict__ trk_ncl = F.in.trk_ncl;
+  const uint32_t n_tracks = F.in.n_tracks;
+  uint32_t* __restrict__ tile_sum = F.at<uint32_t>(F.W.o_tile_sum);
   const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   uint32_t s = 0;
   if (base + SCAN_ITEMS <= n_tracks) {
@@ -56,8 +61,13 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_track_tile_sums(const uint16_t
 }
 
 // single block: exclusive scan of tile_sum in place; tile_sum[n_tiles] = grand total
-__global__ void __launch_bounds__(1024) k_scan_tile_sums(uint32_t* __restrict__ tile_sum, uint32_t n_tiles) {
+template <bool BATCH>
+__global__ void __launch_bounds__(1024) k_scan_tile_sums(const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
   __shared__ uint32_t ws[33];
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
+  uint32_t* __restrict__ tile_sum = F.at<uint32_t>(F.W.o_tile_sum);
+  const uint32_t n_tiles = F.W.n_tiles;
+  if (n_tiles == 0) return;
   uint32_t carry = 0;
   for (uint32_t base = 0; base < n_tiles; base += blockDim.x) {
     uint32_t i = base + threadIdx.x;
@@ -70,10 +80,16 @@ __global__ void __launch_bounds__(1024) k_scan_tile_sums(uint32_t* __restrict__ 
 }
 
 // off[t] for every track; off[n_tracks] = total
-__global__ void __launch_bounds__(SCAN_THREADS) k_track_offsets(const uint16_t* __restrict__ trk_ncl, uint32_t n_tracks,
-                                                               const uint32_t* __restrict__ tile_sum, uint32_t n_tiles,
-                                                               uint32_t* __restrict__ off) {
+template <bool BATCH>
+__global__ void __launch_bounds__(SCAN_THREADS) k_track_offsets(const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
   __shared__ uint32_t ws[33];
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
+  const uint32_t n_tiles = F.W.n_tiles;
+  if (blockIdx.x >= n_tiles) return;
+  const uint16_t* __restrict__ trk_ncl = F.in.trk_ncl;
+  const uint32_t n_tracks = F.in.n_tracks;
+  const uint32_t* __restrict__ tile_sum = F.at<uint32_t>(F.W.o_tile_sum);
+  uint32_t* __restrict__ off = F.at<uint32_t>(F.W.o_off);
   const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
@@ -93,10 +109,14 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_track_offsets(const uint16_t* 
 
 // ---- A4 part 1: column sums over groups of chunks ---------------------------------------------------------------------
 // hist[c][b] (u16) = attached clusters of chunk c in bin b.   gsum[grp][b] = sum over the group's chunks.
-__global__ void __launch_bounds__(256) k_col_group_sums(const uint16_t* __restrict__ hist, uint32_t n_chunks, uint32_t n_bins,
-                                                        uint32_t* __restrict__ gsum) {
+template <bool BATCH>
+__global__ void __launch_bounds__(256) k_col_group_sums(uint32_t n_bins, const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.z);
   const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x, grp = blockIdx.y;
-  if (b >= n_bins) return;
+  const uint32_t n_chunks = F.W.n_chunks;
+  if (b >= n_bins || grp >= F.W.n_groups) return;
+  const uint16_t* __restrict__ hist = F.at<uint16_t>(F.W.o_hist);
+  uint32_t* __restrict__ gsum = F.at<uint32_t>(F.W.o_gsum);
   const uint32_t c0 = grp * COL_GROUP, c1 = min(c0 + COL_GROUP, n_chunks);
   uint32_t s = 0;
 #pragma unroll 8
@@ -105,10 +125,14 @@ __global__ void __launch_bounds__(256) k_col_group_sums(const uint16_t* __restri
 }
 
 // per bin: exclusive scan of gsum over groups (in place), att_cnt[b] = total
-__global__ void __launch_bounds__(256) k_col_group_scan(uint32_t* __restrict__ gsum, uint32_t n_groups, uint32_t n_bins,
-                                                        uint32_t* __restrict__ att_cnt) {
+template <bool BATCH>
+__global__ void __launch_bounds__(256) k_col_group_scan(uint32_t n_bins, const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
   const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= n_bins) return;
+  uint32_t* __restrict__ gsum = F.at<uint32_t>(F.W.o_gsum);
+  uint32_t* __restrict__ att_cnt = F.at<uint32_t>(F.W.o_att_cnt);
+  const uint32_t n_groups = F.W.n_groups;
   uint32_t run = 0;
   uint32_t g = 0;
   for (; g + 8 <= n_groups; g += 8) {
@@ -131,10 +155,14 @@ __global__ void __launch_bounds__(256) k_col_group_scan(uint32_t* __restrict__ g
 
 // single block: bin_offset[b] = exclusive scan of att_cnt[b] + u_cnt[b]; u_start[b] = exclusive scan of u_cnt[b]
 // (C5: a bin holds its attached clusters first, then its unattached ones).  totals[0] = sum u_cnt.
-__global__ void __launch_bounds__(1024) k_bin_offsets(const uint32_t* __restrict__ att_cnt, const uint32_t* __restrict__ u_cnt,
-                                                      uint32_t n_bins, uint32_t* __restrict__ bin_offset,
-                                                      uint32_t* __restrict__ u_start) {
+template <bool BATCH>
+__global__ void __launch_bounds__(1024) k_bin_offsets(uint32_t n_bins, const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
   __shared__ uint32_t ws[33];
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
+  const uint32_t* __restrict__ att_cnt = F.at<uint32_t>(F.W.o_att_cnt);
+  const uint32_t* __restrict__ u_cnt = F.in.u_bin_count;
+  uint32_t* __restrict__ bin_offset = F.bin_offset;
+  uint32_t* __restrict__ u_start = F.at<uint32_t>(F.W.o_u_start);
   const uint32_t per = (n_bins + blockDim.x - 1) / blockDim.x;
   const uint32_t b0 = threadIdx.x * per, b1 = min(b0 + per, n_bins);
   uint32_t sa = 0, su = 0;
@@ -158,11 +186,16 @@ __global__ void __launch_bounds__(1024) k_bin_offsets(const uint32_t* __restrict
 }
 
 // ---- A4 part 2: rel[c][b] = bin_offset[b] + attached clusters of bin b in chunks < c ---------------------------------
-__global__ void __launch_bounds__(256) k_col_apply(const uint16_t* __restrict__ hist, const uint32_t* __restrict__ gsum,
-                                                   const uint32_t* __restrict__ bin_offset, uint32_t n_chunks, uint32_t n_bins,
-                                                   uint32_t* __restrict__ rel) {
+template <bool BATCH>
+__global__ void __launch_bounds__(256) k_col_apply(uint32_t n_bins, const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.z);
   const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x, grp = blockIdx.y;
-  if (b >= n_bins) return;
+  const uint32_t n_chunks = F.W.n_chunks;
+  if (b >= n_bins || grp >= F.W.n_groups) return;
+  const uint16_t* __restrict__ hist = F.at<uint16_t>(F.W.o_hist);
+  const uint32_t* __restrict__ gsum = F.at<uint32_t>(F.W.o_gsum);
+  const uint32_t* __restrict__ bin_offset = F.bin_offset;
+  uint32_t* __restrict__ rel = F.at<uint32_t>(F.W.o_rel);
   const uint32_t c0 = grp * COL_GROUP, c1 = min(c0 + COL_GROUP, n_chunks);
   uint32_t run = bin_offset[b] + gsum[(size_t)grp * n_bins + b];
 #pragma unroll 8

@@ -13,6 +13,7 @@
 #include <cooperative_groups.h>
 
 #include "tmd_common.cuh"
+#include "tmd_rank.cuh"
 #include "tmd_scan.cuh"
 
 namespace tmd {
@@ -54,12 +55,26 @@ constexpr int SC_THREADS = 256;
 constexpr int SC_UNROLL = 4;
 constexpr uint32_t SC_MAX_PER_CTA = (1u << CHUNK_SHIFT_MAX) / SC_CLUSTER;   // 2048 records = 32 KB
 
-// row stride (entries) of the start16 table: n_bins + 1 entries, padded to 16 bytes
-__host__ __device__ inline uint32_t sc_start_stride(uint32_t n_bins) { return (n_bins + 1 + 7) & ~7u; }
 __host__ __device__ inline size_t sc_smem_bytes(uint32_t n_bins) { return (size_t)SC_MAX_PER_CTA * 16 + (size_t)sc_start_stride(n_bins) * 2; }
 
-__global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(DevGeo G, ScatterArgs A) {
+__device__ __forceinline__ ScatterArgs scatter_args(const FrameArgs& F, uint32_t n_bins) {
+  ScatterArgs A;
+  A.inter = F.at<uint2>(F.W.o_inter); A.rank16 = F.at<uint16_t>(F.W.o_rank16); A.rel = F.at<uint32_t>(F.W.o_rel);
+  A.start16 = F.at<uint16_t>(F.W.o_start16);
+  A.a_qtot = F.in.a_qtot; A.a_qmax = F.in.a_qmax; A.a_flags = F.in.a_flags; A.a_sigpad = F.in.a_sigpad; A.a_sigtime = F.in.a_sigtime;
+  A.clusters = F.clusters;
+  A.n_attached = (uint32_t)F.in.n_attached; A.n_clusters_total = (uint32_t)(F.in.n_attached + F.in.n_unattached);
+  A.chunk_shift = F.W.chunk_shift; A.start_stride = sc_start_stride(n_bins);
+  return A;
+}
+
+template <bool BATCH>
+__global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
+                                                           const FrameArgs* __restrict__ table) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
+  if ((blockIdx.x >> SC_CLUSTER_SHIFT) >= F.W.n_chunks) return;     // uniform over the cluster: nobody is left waiting
+  const ScatterArgs A = scatter_args(F, G.n_bins);
   uint4* recs = reinterpret_cast<uint4*>(smem_raw);                                   // this CTA's part of the sorted chunk
   uint16_t* start = reinterpret_cast<uint16_t*>(smem_raw + (size_t)SC_MAX_PER_CTA * 16);  // [n_bins + 1] first slot of every bin
   cg::cluster_group cluster = cg::this_cluster();

@@ -21,11 +21,16 @@ constexpr uint32_t SORT_WINDOW = SORT_THREADS * SORT_ITEMS;
 __device__ __forceinline__ uint32_t len_class(uint32_t ncl) { return ncl < 1024u ? ncl : 1024u + (ncl >> 6); }
 
 // One block per window: shared-memory counting sort by length class, descending.
-__global__ void __launch_bounds__(SORT_THREADS) k_len_sort_window(const uint16_t* __restrict__ trk_ncl, uint32_t n_tracks,
-                                                                  uint32_t* __restrict__ perm) {
+template <bool BATCH>
+__global__ void __launch_bounds__(SORT_THREADS) k_len_sort_window(const __grid_constant__ FrameArgs F0, const FrameArgs* __restrict__ table) {
   __shared__ uint32_t h[LEN_BINS];
   __shared__ uint32_t ws[33];
   static_assert(LEN_BINS == 2 * SORT_THREADS, "two classes per thread");
+  const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
+  const uint32_t n_tracks = F.in.n_tracks;
+  if (blockIdx.x * SORT_WINDOW >= n_tracks) return;
+  const uint16_t* __restrict__ trk_ncl = F.in.trk_ncl;
+  uint32_t* __restrict__ perm = F.at<uint32_t>(F.W.o_perm);
   h[threadIdx.x] = 0;
   h[threadIdx.x + SORT_THREADS] = 0;
   __syncthreads();

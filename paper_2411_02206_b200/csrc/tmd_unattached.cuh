@@ -26,8 +26,19 @@ constexpr int UNATT_ITEMS = 4;
 // One block per bin; tiles of UNATT_THREADS * 4 consecutive clusters, aligned to 4 in the global cluster index so that
 // every stream is read with one vector load per thread (8 B of pad differences, 16 B of time differences, 8 + 8 B of
 // charges, 3 x 4 B of widths / flags); block scan of the per-thread sums with a running carry; 4 x 16-byte stores per thread.
-__global__ void __launch_bounds__(UNATT_THREADS) k_unattached(DevGeo G, UnattachedArgs A) {
+__device__ __forceinline__ UnattachedArgs unattached_args(const FrameArgs& F) {
+  UnattachedArgs A;
+  A.in = F.in; A.u_start = F.at<uint32_t>(F.W.o_u_start); A.bin_offset = F.bin_offset; A.att_cnt = F.at<uint32_t>(F.W.o_att_cnt);
+  A.clusters = F.clusters; A.n_clusters_total = (uint32_t)(F.in.n_attached + F.in.n_unattached);
+  return A;
+}
+
+template <bool BATCH>
+__global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
+                                                              const FrameArgs* __restrict__ table) {
   __shared__ uint32_t ws[33];
+  const UnattachedArgs A = unattached_args(frame_of<BATCH>(F0, table, blockIdx.y));
+  if (A.in.n_unattached == 0) return;
   const uint32_t b = blockIdx.x;
   const uint32_t i0 = A.u_start[b], i1 = A.u_start[b + 1];
   if (i1 == i0) return;

@@ -15,11 +15,12 @@ from . import build as _build
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
-TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT = 0, -1, -2, -3, -4, -5
+TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT, TMD_ERR_DEVICE = 0, -1, -2, -3, -4, -5, -6
 TMD_VALIDATE = 1
 TMD_TIMING = 2
 TMD_SERIAL = 4
 TMD_MAX_KERNELS = 24
+TMD_MAX_BATCH = 1024
 TMD_HOST_SLOTS = 2
 PROBE_FINAL = 0xFFFFFFFF
 
@@ -71,6 +72,8 @@ def lib() -> C.CDLL:
         L.tmd_workspace_bytes.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_uint64, C.POINTER(C.c_size_t)]
         L.tmd_decode.argtypes = [C.c_void_p, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_void_p]
         L.tmd_decode_host.argtypes = L.tmd_decode.argtypes
+        L.tmd_decode_batch.argtypes = [C.c_void_p, C.c_uint32, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_void_p]
+        L.tmd_decode_batch.restype = C.c_int
         L.tmd_destroy.argtypes = [C.c_void_p]
         L.tmd_status_string.argtypes = [C.c_int]
         L.tmd_status_string.restype = C.c_char_p
@@ -80,6 +83,8 @@ def lib() -> C.CDLL:
                                           C.c_size_t, C.c_void_p]
         L.tmd_decode_host_async.argtypes = [C.c_void_p, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_int]
         L.tmd_host_wait.argtypes = [C.c_void_p, C.c_int]
+        L.tmd_selftest_ieee.argtypes = [C.c_uint32, C.POINTER(C.c_uint64)]
+        L.tmd_selftest_ieee.restype = C.c_int
         L.tmd_decode_host_async.restype = C.c_int
         L.tmd_host_wait.restype = C.c_int
         L.tmd_kernel_times.restype = C.c_int
@@ -163,6 +168,20 @@ def tmd_decode(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, 
     _check(lib().tmd_decode(ctx, C.byref(comp), C.byref(out), flags, stream))
 
 
+def make_batch(comps: list, outs: list):
+    """(n_frames, tmd_compressed[n], tmd_output[n]) as contiguous HOST arrays of the structs, for tmd_decode_batch."""
+    assert len(comps) == len(outs) and len(comps) >= 1
+    n = len(comps)
+    ca, oa = (tmd_compressed * n)(*comps), (tmd_output * n)(*outs)
+    return n, ca, oa
+
+
+def tmd_decode_batch(ctx: int, batch, flags: int = 0, stream: int = 0) -> None:
+    """Enqueue the decode of all frames of `batch` (from make_batch) with one launch sequence on CUDA stream `stream`."""
+    n, ca, oa = batch
+    _check(lib().tmd_decode_batch(ctx, n, ca, oa, flags, stream))
+
+
 def tmd_decode_host(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, stream: int = 0) -> None:
     """End-to-end decode with HOST pointers (copies in, decodes, copies out, synchronises)."""
     _check(lib().tmd_decode_host(ctx, C.byref(comp), C.byref(out), flags, stream))
@@ -176,6 +195,13 @@ def tmd_decode_host_async(ctx: int, comp: tmd_compressed, out: tmd_output, flags
 def tmd_host_wait(ctx: int, slot: int = 0) -> None:
     """Block until the frame in pipeline slot `slot` is complete in its host buffers."""
     _check(lib().tmd_host_wait(ctx, slot))
+
+
+def tmd_selftest_ieee(log2_pairs: int = 32) -> tuple[int, int, int]:
+    """Mismatch counts (sqrt, div, floor-clamp) of the kernel's unchecked IEEE sequences against the intrinsics; all 0."""
+    m = (C.c_uint64 * 3)()
+    _check(lib().tmd_selftest_ieee(log2_pairs, m))
+    return int(m[0]), int(m[1]), int(m[2])
 
 
 def tmd_kernel_times(ctx: int) -> list[tuple[str, float]]:

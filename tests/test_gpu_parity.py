@@ -256,3 +256,76 @@ def test_serial_and_timing_flags_do_not_change_the_result():
         assert {"track_decode", "rank", "scatter", "unattached", "bin_offsets"} <= set(times) and all(v >= 0 for v in times.values())
     finally:
         T.tmd_destroy(ctx)
+
+
+def test_batch_of_frames_equals_frame_by_frame():
+    # tmd_decode_batch: frames of very different sizes -- physical events, random bytes, a frame without
+    # tracks, one without unattached clusters, an empty one -- decoded by ONE launch sequence; every frame against the oracle
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    from gpu_util import _as_torch
+    from tmd_inputs.layout import CLUSTER_DTYPE, COMPRESSED_FIELDS
+    geo = build_geometry(36)
+    ev = ph.generate_event(ph.config2_like(1500, 20_000, seed=71), geo)
+    frames = [O.encode(geo, BZ, ev.trk_ncl, ev.trk_qptf, ev.att, ev.leg, ev.un),
+              random_compressed(geo, 3000, 20_000, 72, max_ncl=200), random_compressed(geo, 0, 5000, 73),
+              random_compressed(geo, 700, 0, 74, max_ncl=90), Compressed.empty(0, 0, 0, geo.n_bins),
+              random_compressed(geo, 0, 0, 75, ncl=np.array([65535, 1, 40000, 7], np.uint16)),
+              degenerate_same_bin(geo, np.full(300, 500, np.uint16), 76, n_un=100)]
+    frames += [random_compressed(geo, 50 + 37 * i, 400 * i, 80 + i, max_ncl=30 + 10 * i) for i in range(12)]   # > one table chunk
+    want = [O.decode(geo, BZ, c, probe_step=2) for c in frames]
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        comps, outs, held = [], [], []
+        for i, c in enumerate(frames):
+            dev = {k: _as_torch(np.ascontiguousarray(getattr(c, k))).cuda() for k in COMPRESSED_FIELDS}
+            n = c.n_attached + c.n_unattached
+            d_cl = torch.full((max(n, 1) * 16,), 0xEE, dtype=torch.uint8, device="cuda")
+            d_bo = torch.zeros(geo.n_bins + 1, dtype=torch.int32, device="cuda")
+            d_pr = torch.zeros(max(c.n_tracks, 1) * 6, dtype=torch.int32, device="cuda") if i % 2 == 0 else None   # probes on some frames only
+            ws = torch.empty(T.tmd_workspace_bytes(ctx, c.n_tracks, c.n_attached, c.n_unattached), dtype=torch.uint8, device="cuda")
+            held.append((dev, d_cl, d_bo, d_pr, ws))
+            comps.append(T.make_compressed(dev)); outs.append(T.make_output(d_cl, d_bo, ws, d_pr, 2))
+        T.tmd_decode_batch(ctx, T.make_batch(comps, outs), 0, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for i, (c, (dev, d_cl, d_bo, d_pr, ws), (w_cl, w_bo, w_pr)) in enumerate(zip(frames, held, want)):
+            n = c.n_attached + c.n_unattached
+            got = (d_cl.cpu().numpy()[: n * 16].view(CLUSTER_DTYPE).copy(), d_bo.cpu().numpy().view(np.uint32).copy(),
+                   d_pr.cpu().numpy().view(np.uint32)[: c.n_tracks * 6].reshape(-1, 6).copy() if d_pr is not None else None)
+            assert_same(got, (w_cl, w_bo, w_pr if d_pr is not None else None))
+        with pytest.raises(T.TmdError):                      # TMD_VALIDATE synchronises: not accepted for a batch
+            T.tmd_decode_batch(ctx, T.make_batch(comps, outs), T.TMD_VALIDATE, 0)
+    finally:
+        T.tmd_destroy(ctx)
+
+
+def test_validate_sums_track_lengths_in_64_bits():
+    # 70000 tracks of 65535 clusters sum to 4 587 450 000 = 292 482 704 mod 2^32: an input that declares n_attached =
+    # 292 482 704 must be rejected (a 32-bit sum wraps onto the declared value and the decode would run off the workspace)
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    geo = build_geometry(36)
+    n_trk, n_att = 70_000, 292_482_704
+    assert (n_trk * 65535) % 2 ** 32 == n_att
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    lens = {"n_tracks": n_trk, "n_attached": n_att, "n_residuals": n_att - n_trk, "n_unattached": 0, "n_bins": geo.n_bins}
+    tdt = {"<u2": torch.int16, "i1": torch.int8, "u1": torch.uint8, "<u4": torch.int32}
+    dev = {k: torch.zeros(lens[which], dtype=tdt[dt], device="cuda") for k, (dt, which) in COMPRESSED_FIELDS.items()}
+    dev["trk_ncl"].fill_(-1)                                 # 0xFFFF = 65535
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        out = T.make_output(torch.empty(n_att * 16, dtype=torch.uint8, device="cuda"), torch.empty(geo.n_bins + 1, dtype=torch.int32, device="cuda"),
+                            torch.empty(T.tmd_workspace_bytes(ctx, n_trk, n_att, 0), dtype=torch.uint8, device="cuda"))
+        with pytest.raises(T.TmdError) as e:
+            T.tmd_decode(ctx, T.make_compressed(dev), out, T.TMD_VALIDATE, torch.cuda.current_stream().cuda_stream)
+        assert e.value.status == T.TMD_ERR_CORRUPT
+    finally:
+        T.tmd_destroy(ctx)
+
+
+def test_unchecked_ieee_sequences_equal_the_intrinsics():
+    # the decode kernel's division / square-root fast sequences (no per-operation range check) and its fused
+    # floor-clamp-convert against __fdiv_rn / __fsqrt_rn / floorf + clamp: every sqrt argument of the accepted range,
+    # 2^33 division operand pairs of the accepted ranges (+ edge grid), every pattern for the conversion
+    from paper_2411_02206_b200 import tmd as T
+    assert T.tmd_selftest_ieee(33) == (0, 0, 0)
