@@ -55,8 +55,9 @@ def kernel_algorithmic_bytes(n_trk: int, n_att: int, n_un: int, n_bins: int) -> 
 
 # ------------------------------------------------------------------------------------------------ workload on the device
 def build_workload(name: str, device, seed_offset: int = 0, keep_truth: bool = False):
-    """Synthetic time frame `name` (tmd_inputs.timeframe.WORKLOADS) as device tensors of the compressed SoA.
-    Attached clusters: helix truth -> the library's own encoder (tmd_encode_attached); unattached: compressed domain."""
+    """Synthetic time frame `name` (tmd_inputs.timeframe.WORKLOADS) as device tensors of the compressed SoA: cluster truth
+    (helix tracks + unattached clusters) -> the library's own encoder (tmd_encode_attached + tmd_encode_unattached), itself
+    checked byte for byte against the oracle encoder in the -m gpu tests (bench.py may not run the oracle here)."""
     import torch
     from paper_2411_02206_b200 import tmd as T
     from tmd_inputs import build_geometry, timeframe as tf
@@ -80,21 +81,30 @@ def build_workload(name: str, device, seed_offset: int = 0, keep_truth: bool = F
     ws = torch.empty(T.tmd_workspace_bytes(ctx, n_trk, n_att, 0), dtype=torch.uint8, device=device)
     T.tmd_encode_attached(ctx, truth.trk_ncl, truth.trk_qptf, truth.att, truth.leg, arrays, ws,
                           torch.cuda.current_stream().cuda_stream)
+    del ws
+    un = tf.generate_unattached_truth(geo, n_un, cfg.seed, device, "inv_x", single)
+    n_u = int(un.shape[0])
+    for k in ("u_qtot", "u_qmax", "u_flags", "u_sigpad", "u_sigtime", "u_paddiff", "u_timediff"):
+        arrays[k] = torch.empty(n_u, dtype=tdt[spec[k]], device=device)
+    arrays["u_bin_count"] = torch.empty(geo.n_bins, dtype=torch.int32, device=device)
+    ws = torch.empty(T.tmd_encode_unattached_workspace_bytes(ctx, n_u), dtype=torch.uint8, device=device)
+    T.tmd_encode_unattached(ctx, un, arrays, ws, torch.cuda.current_stream().cuda_stream)
     T.tmd_destroy(ctx)
     del ws
-    if not keep_truth:
+    if keep_truth:
+        truth.un = un
+    else:
         truth = None
-    arrays.update(tf.generate_unattached(geo, n_un, cfg.seed, device, "inv_x", single))
+    del un
     torch.cuda.empty_cache()
     return (geo, arrays, truth) if keep_truth else (geo, arrays)
 
 
 def oracle_sample(workload: str, n_s: int, device):
     """A bounded sample of `workload` for the CPU oracle: the first n_s tracks of the same generator recipe (same pT / length /
-    looper mix) and the same fraction of the unattached clusters.  The attached clusters are ENCODED BY THE ORACLE'S OWN
-    ENCODER -- nothing the oracle reads comes from the CUDA path."""
+    looper mix) and the same fraction of the unattached clusters.  All of them are ENCODED BY THE ORACLE'S OWN ENCODER --
+    nothing the oracle reads comes from the CUDA path."""
     from tmd_inputs import build_geometry, physical as ph, timeframe as tf
-    from tmd_inputs.layout import COMPRESSED_FIELDS, Compressed
     from oracle import tmd_oracle as O
 
     geo = build_geometry(36)
@@ -105,15 +115,10 @@ def oracle_sample(workload: str, n_s: int, device):
     cfg.n_tracks = n_s
     tr = tf.generate_truth(cfg, geo, device, batch=400_000)
     ev_att = tr.att.cpu().numpy().view(ph.CLUSTER_DTYPE).reshape(-1)
+    un = tf.generate_unattached_truth(geo, int(n_un * frac), cfg.seed, device, "inv_x", single)
     comp = O.encode(geo, BZ, tr.trk_ncl.cpu().numpy().view(np.uint16), tr.trk_qptf.cpu().numpy(), ev_att, tr.leg.cpu().numpy(),
-                    np.zeros(0, ph.CLUSTER_DTYPE))
-    del tr, ev_att
-    u = tf.generate_unattached(geo, int(n_un * frac), cfg.seed, device, "inv_x", single)
-    full = Compressed.empty(comp.n_tracks, comp.n_attached, int(u["u_qtot"].shape[0]), geo.n_bins)
-    for k, (dt, _) in COMPRESSED_FIELDS.items():
-        src = u[k].cpu().numpy().view(np.dtype(dt)) if k in u else getattr(comp, k)
-        getattr(full, k)[:] = src
-    return geo, full, n_s
+                    un.cpu().numpy().view(ph.CLUSTER_DTYPE).reshape(-1))
+    return geo, comp, n_s
 
 
 def time_oracle(geo, comp) -> float:

@@ -245,6 +245,20 @@ typedef struct {
 int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compressed* out, void* workspace, size_t workspace_bytes,
                         void* cuda_stream);
 
+/*
+ * Track-model ENCODING of the unattached clusters ("unassigned clusters are sorted by coordinate position
+ * ... stored as differences relative to the preceding cluster"): per (sector,row) bin, sort ascending
+ * by the tuple (time, pad, qtot, qmax, sigpad, sigtime, flags), store pad / time as differences to the predecessor (first
+ * of a bin: to (0,0)), copy the other fields through.  `un` = DEVICE array of n_unattached clusters in ANY order (sector
+ * and row name the bin).  Writes out->u_bin_count [n_sectors_out * n_rows] and the seven u_* arrays [n_unattached] (as
+ * writable DEVICE memory; every other member of `out` is ignored).  `workspace` >= tmd_encode_unattached_workspace_bytes,
+ * 256-byte aligned.  Synchronises the stream.  TMD_ERR_CORRUPT if a cluster's row / sector has no output bin.
+ * With tmd_encode_attached this is the whole encoder: tmd_decode(encode(x)) reproduces x in canonical order.
+ */
+int tmd_encode_unattached_workspace_bytes(const tmd_ctx* ctx, uint64_t n_unattached, size_t* out_bytes);
+int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster* un, tmd_compressed* out, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -7,6 +7,7 @@
 #include "tmd_common.cuh"
 #include "tmd_decode.cuh"
 #include "tmd_encode.cuh"
+#include "tmd_encode_unattached.cuh"
 #include "tmd_rank.cuh"
 #include "tmd_scan.cuh"
 #include "tmd_scatter.cuh"
@@ -81,6 +82,8 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att, int n_sm) {
   w.o_rank16 = take((size_t)n_att * 2);
   w.o_inter = take((size_t)n_att * 8);
   w.o_table = take((size_t)TMD_MAX_BATCH * sizeof(FrameArgs));   // the frame table of a batch lives in frame 0's workspace
+  w.n_sort_words = ((n_tracks + SORT_WINDOW - 1) / SORT_WINDOW) * LEN_BINS;     // key histograms of the track sort (A2)
+  w.o_sort_hist = take((size_t)w.n_sort_words * 4);
   w.total = o;
   return w;
 }
@@ -200,7 +203,7 @@ struct Launcher {
 // The launch sequence of rows A1-A7 over `n_frames` frames.  BATCH = false: one frame, its FrameArgs
 // passed by value.  BATCH = true: the frames' FrameArgs are in device memory (`table`) and every grid has a frame
 // coordinate; `mx` holds the per-kernel maxima of the frames' grid extents.
-struct Extents { uint32_t n_tiles, n_tracks, n_chunks, n_groups; bool any_probe; };
+struct Extents { uint32_t n_tiles, n_tracks, n_chunks, n_groups; uint64_t n_unattached; bool any_probe; };
 
 template <bool BATCH>
 int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t n_frames, const Extents& mx, Launcher& L) {
@@ -214,8 +217,10 @@ int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t 
     TMD_LAUNCH("scan_tile_sums", k_scan_tile_sums<BATCH><<<dim3(1, nf), 1024, 0, st>>>(F0, table));
     TMD_LAUNCH("track_offsets", k_track_offsets<BATCH><<<dim3(mx.n_tiles, nf), SCAN_THREADS, 0, st>>>(F0, table));
     // A2: load-balance order (counting sort by cluster count, longest first, inside windows of consecutive tracks)
-    TMD_LAUNCH("len_sort_window",
-               k_len_sort_window<BATCH><<<dim3((mx.n_tracks + SORT_WINDOW - 1) / SORT_WINDOW, nf), SORT_THREADS, 0, st>>>(F0, table));
+    const uint32_t sort_blocks = (mx.n_tracks + SORT_BLOCK_TRACKS - 1) / SORT_BLOCK_TRACKS, sort_windows = (mx.n_tracks + SORT_WINDOW - 1) / SORT_WINDOW;
+    TMD_LAUNCH("sort_count", k_sort_count<BATCH><<<dim3(sort_blocks, nf), SORT_THREADS, 0, st>>>(F0, table));
+    TMD_LAUNCH("sort_scan", k_sort_scan<BATCH><<<dim3(sort_windows, nf), SORT_THREADS, 0, st>>>(F0, table));
+    TMD_LAUNCH("sort_place", k_sort_place<BATCH><<<dim3(sort_blocks, nf), SORT_THREADS, 0, st>>>(F0, table));
     // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
     const dim3 dg((mx.n_tracks + DECODE_THREADS - 1) / DECODE_THREADS, nf);
     if (mx.any_probe) TMD_LAUNCH("track_decode", k_track_decode<true, BATCH><<<dg, DECODE_THREADS, ctx->decode_smem, st>>>(G, F0, table));
@@ -238,7 +243,9 @@ int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t 
   if (mx.n_tracks > 0)
     TMD_LAUNCH("col_apply", k_col_apply<BATCH><<<dim3(bin_blocks, mx.n_groups, nf), 256, 0, st>>>(n_bins, F0, table));
   // A7: unattached clusters
-  TMD_LAUNCH("unattached", k_unattached<BATCH><<<dim3(n_bins, nf), UNATT_THREADS, 0, st>>>(G, F0, table));
+  // A7: unattached clusters; a block per bin for full time frames, a warp per bin where bins hold few clusters
+  const uint32_t un_bpb = mx.n_unattached / n_bins >= 512 ? 1u : (uint32_t)UNATT_WARPS;
+  TMD_LAUNCH("unattached", k_unattached<BATCH><<<dim3((n_bins + un_bpb - 1) / un_bpb, nf), UNATT_THREADS, 0, st>>>(G, F0, table, un_bpb));
   if (mx.n_tracks > 0) {
     // A6: copy-through + scatter (a thread-block cluster of SC_CLUSTER CTAs per chunk)
     cudaLaunchConfig_t cfg = {};
@@ -437,7 +444,7 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
   }
   Launcher L{ctx, st, timing};
-  const Extents mx = {F.W.n_tiles, in->n_tracks, F.W.n_chunks, F.W.n_groups, out->probe_state != nullptr};
+  const Extents mx = {F.W.n_tiles, in->n_tracks, F.W.n_chunks, F.W.n_groups, in->n_unattached, out->probe_state != nullptr};
   rc = enqueue<false>(ctx, F, nullptr, 1, mx, L);
   ctx->launches = L.n + (validate ? 1 : 0);
   if (rc != TMD_OK) return rc;
@@ -460,7 +467,7 @@ int tmd_decode_batch(tmd_ctx* ctx, uint32_t n_frames, const tmd_compressed* in, 
   const bool timing = (flags & TMD_TIMING) != 0;
   int rc = prepare_timing(ctx, timing);
   if (rc != TMD_OK) return rc;
-  Extents mx = {0, 0, 0, 0, false};
+  Extents mx = {0, 0, 0, 0, 0, false};
   FrameArgs* table = nullptr;
   FrameChunk chunk;
   // Chunk size of the batch: the one a single frame holding ALL the attached clusters would get (larger than any
@@ -488,6 +495,7 @@ int tmd_decode_batch(tmd_ctx* ctx, uint32_t n_frames, const tmd_compressed* in, 
     mx.n_tracks = mx.n_tracks > in[i].n_tracks ? mx.n_tracks : in[i].n_tracks;
     mx.n_chunks = mx.n_chunks > F.W.n_chunks ? mx.n_chunks : F.W.n_chunks;
     mx.n_groups = mx.n_groups > F.W.n_groups ? mx.n_groups : F.W.n_groups;
+    mx.n_unattached = mx.n_unattached > in[i].n_unattached ? mx.n_unattached : in[i].n_unattached;
     mx.any_probe = mx.any_probe || out[i].probe_state != nullptr;
   }
   Launcher L{ctx, st, timing};
@@ -559,6 +567,88 @@ int tmd_encode_attached(tmd_ctx* ctx, const tmd_attached_truth* in, tmd_compress
   if (cudaMemcpyAsync(&h_err[ERR_WORDS], d_off + in->n_tracks, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TMD_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return TMD_ERR_CUDA;
   if (h_err[ERR_TRACK_FIELD] || h_err[ERR_WORDS] != (uint32_t)in->n_attached) return TMD_ERR_CORRUPT;
+  return TMD_OK;
+}
+
+namespace {
+struct UnWorkspace { size_t o_err, o_bin_start, o_tile_start, o_cursor, o_max_tiles, o_buf_a, o_buf_b, total; };
+UnWorkspace un_layout(uint32_t n_bins, uint64_t n_un) {
+  UnWorkspace w;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
+  w.o_err = take(ERR_WORDS * 4);
+  w.o_bin_start = take(((size_t)n_bins + 1) * 4);
+  w.o_tile_start = take(((size_t)n_bins + 1) * 4);
+  w.o_cursor = take((size_t)n_bins * 4);
+  w.o_max_tiles = take(4);
+  w.o_buf_a = take((size_t)n_un * 16);
+  w.o_buf_b = take((size_t)n_un * 16);
+  w.total = o;
+  return w;
+}
+}  // namespace
+
+int tmd_encode_unattached_workspace_bytes(const tmd_ctx* ctx, uint64_t n_unattached, size_t* out_bytes) {
+  if (!ctx || !out_bytes || n_unattached > TMD_MAX_CLUSTERS) return TMD_ERR_ARG;
+  *out_bytes = un_layout(ctx->geo.n_bins, n_unattached).total;
+  return TMD_OK;
+}
+
+int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster* un, tmd_compressed* out, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream) {
+  if (!ctx || !out || n_unattached > TMD_MAX_CLUSTERS || !out->u_bin_count) return TMD_ERR_ARG;
+  if (n_unattached > 0 && (!un || !out->u_qtot || !out->u_qmax || !out->u_flags || !out->u_sigpad || !out->u_sigtime || !out->u_paddiff ||
+                           !out->u_timediff))
+    return TMD_ERR_ARG;
+  if (misaligned(un, 16)) return TMD_ERR_ALIGN;
+  const uint32_t n_bins = ctx->geo.n_bins, n_un = (uint32_t)n_unattached;
+  const UnWorkspace W = un_layout(n_bins, n_unattached);
+  if (!workspace || workspace_bytes < W.total) return TMD_ERR_WORKSPACE;
+  if (misaligned(workspace, ALIGN)) return TMD_ERR_ALIGN;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)workspace;
+  UnEncodeArgs A;
+  A.n_un = n_un; A.n_bins = n_bins; A.n_rows = ctx->geo.n_rows;
+  A.un = (const uint4*)un;
+  A.bin_count = (uint32_t*)out->u_bin_count;
+  A.bin_start = (uint32_t*)(ws + W.o_bin_start); A.tile_start = (uint32_t*)(ws + W.o_tile_start);
+  A.cursor = (uint32_t*)(ws + W.o_cursor); A.max_tiles = (uint32_t*)(ws + W.o_max_tiles);
+  A.buf_a = (uint4*)(ws + W.o_buf_a); A.buf_b = (uint4*)(ws + W.o_buf_b);
+  uint32_t* d_err = (uint32_t*)(ws + W.o_err);
+  TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
+  TMD_CUDA(cudaMemsetAsync(A.bin_count, 0, (size_t)n_bins * 4, st));
+  const uint32_t stream_blocks = (uint32_t)ctx->n_sm * 8;
+  if (n_un > 0) k_un_count<<<stream_blocks, 256, 0, st>>>(A, d_err);
+  k_un_offsets<<<1, 1024, 0, st>>>(A);
+  TMD_CUDA(cudaGetLastError());
+  uint32_t h_err[ERR_WORDS], h_max_tiles = 0;
+  TMD_CUDA(cudaMemcpyAsync(h_err, d_err, sizeof(h_err), cudaMemcpyDeviceToHost, st));
+  TMD_CUDA(cudaMemcpyAsync(&h_max_tiles, A.max_tiles, 4, cudaMemcpyDeviceToHost, st));
+  TMD_CUDA(cudaStreamSynchronize(st));
+  if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;       // a row / sector without an output bin
+  if (n_un == 0) return TMD_OK;
+  static bool smem_set = false;
+  if (!smem_set) {
+    TMD_CUDA(allow_smem(k_un_sort_tiles, (size_t)UN_TILE * 16));
+    TMD_CUDA(allow_smem(k_un_merge, (size_t)UN_TILE * 16));
+    smem_set = true;
+  }
+  const uint32_t tile_bound = n_un / UN_TILE + n_bins;      // >= number of tiles; surplus blocks return at once
+  k_un_bucket<<<stream_blocks, 256, 0, st>>>(A);
+  k_un_sort_tiles<<<tile_bound, UN_THREADS, (size_t)UN_TILE * 16, st>>>(A);
+  const uint4* src = A.buf_a;
+  uint4* dst = A.buf_b;
+  for (uint32_t p = 0; (1u << p) < h_max_tiles; ++p) {      // runs of 2^p tiles -> runs of 2^(p+1) tiles
+    k_un_merge<<<tile_bound, UN_THREADS, (size_t)UN_TILE * 16, st>>>(A, src, dst, p);
+    const uint4* t = src; src = dst; dst = (uint4*)t;
+  }
+  UnDiffOut O;
+  O.u_qtot = (uint16_t*)out->u_qtot; O.u_qmax = (uint16_t*)out->u_qmax; O.u_flags = (uint8_t*)out->u_flags;
+  O.u_sigpad = (uint8_t*)out->u_sigpad; O.u_sigtime = (uint8_t*)out->u_sigtime;
+  O.u_paddiff = (uint16_t*)out->u_paddiff; O.u_timediff = (uint32_t*)out->u_timediff;
+  k_un_diff<<<stream_blocks, 256, 0, st>>>(A, src, O);
+  TMD_CUDA(cudaGetLastError());
+  TMD_CUDA(cudaStreamSynchronize(st));
   return TMD_OK;
 }
 

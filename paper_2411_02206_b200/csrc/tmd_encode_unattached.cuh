@@ -38,7 +38,8 @@ __device__ __forceinline__ UnKey un_key(const uint4& r) {
   k.k0 = r.x;                                                          // time
   k.k1 = (r.y << 16) | (r.y >> 16);                                    // pad : qtot
   k.k2 = ((r.z & 0xFFFFu) << 16) | ((r.z >> 8) & 0xFF00u) | (r.z >> 24);   // qmax : sigpad : sigtime
-  k.k3 = r.w & 0xFFu;                                                  // flags
+  k.k3 = (r.w << 24) | (r.w >> 8);                                     // flags, then (row, sector, zero): equal inside a bin, and
+                                                                       // below the all-ones padding record of a partial tile
   return k;
 }
 __device__ __forceinline__ bool un_less(const uint4& a, const uint4& b) {

@@ -21,11 +21,10 @@ struct UnattachedArgs {
 };
 
 constexpr int UNATT_THREADS = 256;
+constexpr int UNATT_WARPS = UNATT_THREADS / 32;
 constexpr int UNATT_ITEMS = 4;
+constexpr uint32_t UNATT_SMALL = 1024;     // bins up to this many clusters are decoded by one warp, larger ones by the block
 
-// One block per bin; tiles of UNATT_THREADS * 4 consecutive clusters, aligned to 4 in the global cluster index so that
-// every stream is read with one vector load per thread (8 B of pad differences, 16 B of time differences, 8 + 8 B of
-// charges, 3 x 4 B of widths / flags); block scan of the per-thread sums with a running carry; 4 x 16-byte stores per thread.
 __device__ __forceinline__ UnattachedArgs unattached_args(const FrameArgs& F) {
   UnattachedArgs A;
   A.in = F.in; A.u_start = F.at<uint32_t>(F.W.o_u_start); A.bin_offset = F.bin_offset; A.att_cnt = F.at<uint32_t>(F.W.o_att_cnt);
@@ -33,13 +32,11 @@ __device__ __forceinline__ UnattachedArgs unattached_args(const FrameArgs& F) {
   return A;
 }
 
-template <bool BATCH>
-__global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
-                                                              const FrameArgs* __restrict__ table) {
-  __shared__ uint32_t ws[33];
-  const UnattachedArgs A = unattached_args(frame_of<BATCH>(F0, table, blockIdx.y));
-  if (A.in.n_unattached == 0) return;
-  const uint32_t b = blockIdx.x;
+// Decode bin b with NT cooperating threads (thread index `tid` in 0..NT-1): NT = 32 is one warp (shuffle scan, no block
+// barrier), NT = UNATT_THREADS the whole block (NT is uniform over the calling warp, and over the block when it is the block).  Tiles of NT * 4 consecutive clusters, aligned to 4 in the global cluster
+// index so that every stream is read with one vector load per thread (8 B of pad differences, 16 B of time differences,
+// 8 + 8 B of charges, 3 x 4 B of widths / flags); scan of the per-thread sums with a running carry; 4 x 16-byte stores per thread.
+__device__ __forceinline__ void unattached_bin(const DevGeo& G, const UnattachedArgs& A, uint32_t b, uint32_t tid, const uint32_t NT, uint32_t* ws) {
   const uint32_t i0 = A.u_start[b], i1 = A.u_start[b + 1];
   if (i1 == i0) return;
   const uint32_t n_un = (uint32_t)A.in.n_unattached;
@@ -47,8 +44,8 @@ __global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_const
   const uint32_t sec = b / G.n_rows, row = b - sec * G.n_rows;
   const uint32_t tail = (row << 8) | (sec << 16);
   uint32_t carry_p = 0, carry_t = 0;
-  for (uint32_t base = i0 & ~3u; base < i1; base += UNATT_THREADS * UNATT_ITEMS) {
-    const uint32_t k0 = base + threadIdx.x * UNATT_ITEMS;        // multiple of 4
+  for (uint32_t base = i0 & ~3u; base < i1; base += NT * UNATT_ITEMS) {
+    const uint32_t k0 = base + tid * UNATT_ITEMS;        // multiple of 4
     uint32_t pd[4] = {0, 0, 0, 0}, td[4] = {0, 0, 0, 0}, qt[4], qm[4], sp[4], st[4], fl[4];
     if (k0 < i1 && k0 + 4 > i0) {
       if (k0 + 4 <= n_un) {
@@ -83,9 +80,15 @@ __global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_const
       pd[k] = sum_p;
       td[k] = sum_t;
     }
-    uint32_t tot_p, tot_t;
-    const uint32_t ex_p = carry_p + block_excl_scan(sum_p, ws, &tot_p);
-    const uint32_t ex_t = carry_t + block_excl_scan(sum_t, ws, &tot_t);
+    uint32_t tot_p, tot_t, ex_p, ex_t;
+    if (NT == 32) {
+      const uint32_t inc_p = warp_incl_scan(sum_p), inc_t = warp_incl_scan(sum_t);
+      tot_p = __shfl_sync(0xffffffffu, inc_p, 31); tot_t = __shfl_sync(0xffffffffu, inc_t, 31);
+      ex_p = carry_p + inc_p - sum_p; ex_t = carry_t + inc_t - sum_t;
+    } else {
+      ex_p = carry_p + block_excl_scan(sum_p, ws, &tot_p);
+      ex_t = carry_t + block_excl_scan(sum_t, ws, &tot_t);
+    }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       const uint32_t i = k0 + k;
@@ -100,6 +103,25 @@ __global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_const
     }
     carry_p += tot_p;
     carry_t += tot_t;
+  }
+}
+
+// A block owns `bins_per_block` consecutive bins (1 for full time frames, UNATT_WARPS for frames with few clusters per
+// bin: single events, batches of small frames).  Bins with more than UNATT_SMALL clusters are decoded by the whole block,
+// one after the other (the decision is uniform over the block); the others by one warp each.
+template <bool BATCH>
+__global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
+                                                              const FrameArgs* __restrict__ table, uint32_t bins_per_block) {
+  __shared__ uint32_t ws[33];
+  const UnattachedArgs A = unattached_args(frame_of<BATCH>(F0, table, blockIdx.y));
+  if (A.in.n_unattached == 0) return;
+  const uint32_t b0 = blockIdx.x * bins_per_block, b1 = min(b0 + bins_per_block, G.n_bins);
+  const uint32_t wid = threadIdx.x >> 5, lane = lane_id();
+  for (uint32_t b = b0; b < b1; ++b) {
+    const uint32_t n = A.u_start[b + 1] - A.u_start[b];
+    const bool whole_block = n > UNATT_SMALL;
+    if (whole_block || (b - b0) % UNATT_WARPS == wid)
+      unattached_bin(G, A, b, whole_block ? threadIdx.x : lane, whole_block ? (uint32_t)UNATT_THREADS : 32u, ws);
   }
 }
 

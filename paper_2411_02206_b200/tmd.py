@@ -83,6 +83,10 @@ def lib() -> C.CDLL:
                                           C.c_size_t, C.c_void_p]
         L.tmd_decode_host_async.argtypes = [C.c_void_p, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_int]
         L.tmd_host_wait.argtypes = [C.c_void_p, C.c_int]
+        L.tmd_encode_unattached_workspace_bytes.argtypes = [C.c_void_p, C.c_uint64, C.POINTER(C.c_size_t)]
+        L.tmd_encode_unattached_workspace_bytes.restype = C.c_int
+        L.tmd_encode_unattached.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.POINTER(tmd_compressed), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.tmd_encode_unattached.restype = C.c_int
         L.tmd_selftest_ieee.argtypes = [C.c_uint32, C.POINTER(C.c_uint64)]
         L.tmd_selftest_ieee.restype = C.c_int
         L.tmd_decode_host_async.restype = C.c_int
@@ -223,3 +227,21 @@ def tmd_encode_attached(ctx: int, trk_ncl, trk_qptf, att, leg, out_arrays: dict,
             setattr(c, k, _ptr(out_arrays[k]))
     ws_bytes = int(workspace.numel() * workspace.element_size())
     _check(lib().tmd_encode_attached(ctx, C.byref(truth), C.byref(c), _ptr(workspace), ws_bytes, stream))
+
+
+def tmd_encode_unattached_workspace_bytes(ctx: int, n_unattached: int) -> int:
+    out = C.c_size_t()
+    _check(lib().tmd_encode_unattached_workspace_bytes(ctx, n_unattached, C.byref(out)))
+    return out.value
+
+
+def tmd_encode_unattached(ctx: int, un, out_arrays: dict, workspace, stream: int = 0) -> None:
+    """Encode unattached clusters (DEVICE tensor of 16-byte records, any order) into the u_* arrays and u_bin_count of
+    `out_arrays` (DEVICE, writable)."""
+    n = int(un.shape[0])
+    c = tmd_compressed(0, 0, n)
+    for k, _ in COMPRESSED_ARRAYS:
+        if k in out_arrays:
+            setattr(c, k, _ptr(out_arrays[k]))
+    ws_bytes = int(workspace.numel() * workspace.element_size())
+    _check(lib().tmd_encode_unattached(ctx, n, _ptr(un), C.byref(c), _ptr(workspace), ws_bytes, stream))

@@ -7,7 +7,8 @@ A full time frame (c3: 251 M attached + 80 M unattached clusters) is more than t
    fixes at any size -- `decode(encode(x)) == canonical(x)` (pinned for the oracle at small sizes in
    test_oracle_roundtrip.py): `bin_offset` is the exclusive cumsum of the per-bin counts of the generator's clusters, the
    attached part of every bin is the generator's clusters in a stable sort by bin, the unattached
-   part is the per-bin cumulative sum of the stored differences (C4).  No expected value comes from the CUDA path.
+   part is the generator's unattached clusters of the bin sorted by the encoder's tuple (C6).  No expected value comes from
+   the CUDA path.
 2. SAMPLED tracks (random ones, the longest ones, the first and the last) go through the ORACLE one by one: the oracle's
    encoder, fed with the generator's clusters of the track, must produce the bytes the GPU encoder left in the workload
    (so the oracle's input is its own), and the oracle's decode of them must equal the records the GPU wrote at the
@@ -66,25 +67,26 @@ def test_full_time_frame(name):
     bad = (got[dest] != truth.att).any(dim=1)
     assert not bool(bad.any()), f"{int(bad.sum())} attached records differ; first g = {int(bad.nonzero()[0])}"
     del bad
-    # unattached: per-bin running sums of the stored differences (C4), appended after the bin's attached clusters
-    ubin = torch.repeat_interleave(torch.arange(n_bins, device=dev), u_cnt)
-    first = u_start[ubin]
-    i_in = torch.arange(n_un, device=dev) - first
-    cp = torch.cumsum(arrays["u_paddiff"].to(torch.int64) & 0xFFFF, 0)
-    ct = torch.cumsum(arrays["u_timediff"].to(torch.int64) & 0xFFFFFFFF, 0)
-    zero = torch.zeros(1, dtype=torch.int64, device=dev)
-    before_p = torch.cat((zero, cp))[first]
-    before_t = torch.cat((zero, ct))[first]
-    pad = (cp - before_p) & 0xFFFF
-    time = (ct - before_t) & 0xFFFFFFFF
-    del cp, ct, before_p, before_t
-    want_u = tf.pack_records(time, pad, arrays["u_qtot"].to(torch.int64) & 0xFFFF, arrays["u_qmax"].to(torch.int64) & 0xFFFF,
-                             arrays["u_sigpad"].to(torch.int64), arrays["u_sigtime"].to(torch.int64),
-                             arrays["u_flags"].to(torch.int64), ubin % geo.n_rows, ubin // geo.n_rows)
+    # unattached: the generator's clusters in the encoder's order -- per bin ascending by (time, pad, qtot, qmax, sigpad,
+    # sigtime, flags) (C6), two stable library sorts -- appended after the bin's attached clusters (C5)
+    un = truth.un.to(torch.int64)
+    u0, u1, u2, u3 = (un[:, k] & 0xFFFFFFFF for k in range(4))
+    ubin_any = ((u3 >> 16) & 0xFF) * geo.n_rows + ((u3 >> 8) & 0xFF)
+    assert torch.equal(torch.bincount(ubin_any, minlength=n_bins), u_cnt), "u_bin_count"
+    key_lo = ((u1 >> 16) << 40) | ((u2 & 0xFFFF) << 24) | (((u2 >> 16) & 0xFF) << 16) | (((u2 >> 24) & 0xFF) << 8) | (u3 & 0xFF)
+    key_hi = (ubin_any << 48) | (u0 << 16) | (u1 & 0xFFFF)
+    o1 = torch.sort(key_lo, stable=True).indices
+    o2 = torch.sort(key_hi[o1], stable=True).indices
+    order_u = o1[o2]
+    del un, u0, u1, u2, u3, key_lo, key_hi, o1, o2
+    want_u = truth.un[order_u]
+    ubin = ubin_any[order_u]
+    del order_u, ubin_any
+    i_in = torch.arange(n_un, device=dev) - u_start[ubin]
     udest = want_bo[ubin] + att_cnt[ubin] + i_in
     bad = (got[udest] != want_u).any(dim=1)
     assert not bool(bad.any()), f"{int(bad.sum())} unattached records differ"
-    del bad, want_u, udest, ubin, first, i_in, pad, time
+    del bad, want_u, udest, ubin, i_in
 
     # ---- 2. sampled tracks through the oracle, one by one
     rng = np.random.default_rng(7)

@@ -181,25 +181,20 @@ def test_gpu_encoder_matches_oracle_encoder(phys_case):
 
 
 def test_bench_workload_builder_matches_oracle():
-    # the path bench.py times: torch helix truth -> GPU encoder -> GPU decoder.  The oracle gets the generator's clusters
-    # and its OWN encoder's bytes; the GPU encoder's bytes must be the same, then both decoders must agree.
+    # the path bench.py times: torch cluster truth -> GPU encoder (attached + unattached) -> GPU decoder.  The oracle gets the
+    # generator's clusters and its OWN encoder's bytes; the GPU encoder's bytes must be the same, then both decoders must agree.
     import torch
     import bench
     from tmd_inputs.layout import CLUSTER_DTYPE, COMPRESSED_FIELDS
     geo, arrays, truth = bench.build_workload("c1", torch.device("cuda", 0), keep_truth=True)
     att = truth.att.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1)
     comp = O.encode(geo, BZ, truth.trk_ncl.cpu().numpy().view(np.uint16), truth.trk_qptf.cpu().numpy(), att, truth.leg.cpu().numpy(),
-                    np.zeros(0, CLUSTER_DTYPE))
-    assert comp.n_tracks == 10_000 and 1.1e6 < comp.n_attached < 1.4e6
-    full = Compressed.empty(comp.n_tracks, comp.n_attached, int(arrays["u_qtot"].shape[0]), geo.n_bins)
+                    truth.un.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1))
+    assert comp.n_tracks == 10_000 and 1.1e6 < comp.n_attached < 1.4e6 and 2.9e5 < comp.n_unattached < 3.1e5
     for k, (dt, which) in COMPRESSED_FIELDS.items():
         mine = arrays[k].cpu().numpy().view(np.dtype(dt))
-        if which in ("n_tracks", "n_attached", "n_residuals"):
-            assert np.array_equal(mine, getattr(comp, k)), f"GPU encoder, {k}: " + first_mismatch(mine, getattr(comp, k))
-            getattr(full, k)[:] = getattr(comp, k)
-        else:
-            getattr(full, k)[:] = mine                    # unattached: drawn in the compressed domain by the generator
-    assert_same(gpu_decode(geo, BZ, full, probe_step=0xFFFFFFFF), O.decode(geo, BZ, full, probe_step=0xFFFFFFFF))
+        assert np.array_equal(mine, getattr(comp, k)), f"GPU encoder, {k}: " + first_mismatch(mine, getattr(comp, k))
+    assert_same(gpu_decode(geo, BZ, comp, probe_step=0xFFFFFFFF), O.decode(geo, BZ, comp, probe_step=0xFFFFFFFF))
 
 
 def test_pipelined_host_entry_points_match():
@@ -252,7 +247,7 @@ def test_serial_and_timing_flags_do_not_change_the_result():
                             torch.empty(T.tmd_workspace_bytes(ctx, c.n_tracks, c.n_attached, c.n_unattached), dtype=torch.uint8, device="cuda"))
         T.tmd_decode(ctx, T.make_compressed(dev), out, T.TMD_TIMING | T.TMD_SERIAL, torch.cuda.current_stream().cuda_stream)
         times = dict(T.tmd_kernel_times(ctx))
-        assert T.tmd_last_launch_count(ctx) == len(times) == 12
+        assert T.tmd_last_launch_count(ctx) == len(times) == 14
         assert {"track_decode", "rank", "scatter", "unattached", "bin_offsets"} <= set(times) and all(v >= 0 for v in times.values())
     finally:
         T.tmd_destroy(ctx)
@@ -329,3 +324,79 @@ def test_unchecked_ieee_sequences_equal_the_intrinsics():
     # 2^33 division operand pairs of the accepted ranges (+ edge grid), every pattern for the conversion
     from paper_2411_02206_b200 import tmd as T
     assert T.tmd_selftest_ieee(33) == (0, 0, 0)
+
+
+def _gpu_encode_unattached(geo, un):
+    """tmd_encode_unattached on numpy cluster records -> dict of numpy arrays (u_* and u_bin_count)."""
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        n = len(un)
+        d_un = torch.from_numpy(np.ascontiguousarray(un).view(np.int32).reshape(-1, 4).copy()).cuda()
+        tdt = {"<u2": torch.int16, "i1": torch.int8, "u1": torch.uint8, "<u4": torch.int32}
+        out = {k: torch.full((n if w == "n_unattached" else geo.n_bins,), -1, dtype=tdt[dt], device="cuda")
+               for k, (dt, w) in COMPRESSED_FIELDS.items() if k.startswith("u_")}
+        ws = torch.empty(T.tmd_encode_unattached_workspace_bytes(ctx, n), dtype=torch.uint8, device="cuda")
+        T.tmd_encode_unattached(ctx, d_un, out, ws, torch.cuda.current_stream().cuda_stream)
+        return {k: v.cpu().numpy().view(np.dtype(COMPRESSED_FIELDS[k][0])) for k, v in out.items()}
+    finally:
+        T.tmd_destroy(ctx)
+
+
+def _assert_unattached_encoding_equals_oracle(geo, un):
+    from tmd_inputs.layout import CLUSTER_DTYPE
+    want = O.encode(geo, BZ, np.zeros(0, np.uint16), np.zeros(0, np.float32), np.zeros(0, CLUSTER_DTYPE), np.zeros(0, np.uint8), un)
+    got = _gpu_encode_unattached(geo, un)
+    for k, v in got.items():
+        assert np.array_equal(v, getattr(want, k)), f"{k}: " + first_mismatch(v, getattr(want, k))
+
+
+def test_gpu_unattached_encoder_matches_oracle_encoder(phys_case):
+    # PAPER.md L68: "unassigned clusters are sorted by coordinate position ... stored as differences relative to the preceding
+    # cluster": the library's per-bin sort + differencing produces the oracle encoder's bytes
+    name, geo, ev, comp = phys_case
+    got = _gpu_encode_unattached(geo, ev.un)
+    for k, v in got.items():
+        assert np.array_equal(v, getattr(comp, k)), f"{k}: " + first_mismatch(v, getattr(comp, k))
+
+
+def test_gpu_unattached_encoder_ties_skew_and_empty():
+    from tmd_inputs.layout import CLUSTER_DTYPE
+    geo = build_geometry(36)
+    rng = np.random.default_rng(91)
+    # (a) heavy ties: few distinct times / pads / charges, so that the order is decided deep in the tuple, with exact duplicates
+    n = 400_000
+    un = np.zeros(n, CLUSTER_DTYPE)
+    b = rng.integers(0, 40, n)                                  # 40 bins of ~10 000 clusters: several tiles per bin
+    un["sector"], un["row"] = b // 8, 17 + b % 8
+    un["time"] = rng.integers(0, 50, n); un["pad"] = rng.integers(0, 3, n); un["qtot"] = rng.integers(0, 2, n)
+    un["qmax"] = rng.integers(0, 2, n); un["sigpad"] = rng.integers(0, 2, n); un["sigtime"] = rng.integers(0, 2, n)
+    un["flags"] = rng.integers(0, 3, n)
+    _assert_unattached_encoding_equals_oracle(geo, un)
+    # (b) one bin far larger than a tile (eight merge passes), extreme values (the all-ones record equals the tile padding key)
+    n = 300_000
+    un = np.zeros(n, CLUSTER_DTYPE)
+    un["sector"], un["row"] = 35, 151
+    un["time"] = rng.integers(0, 2 ** 32, n); un["pad"] = rng.integers(0, 65536, n); un["qtot"] = rng.integers(0, 65536, n)
+    un["qmax"] = rng.integers(0, 65536, n); un["sigpad"] = rng.integers(0, 256, n); un["sigtime"] = rng.integers(0, 256, n)
+    un["flags"] = rng.integers(0, 256, n)
+    for f, v in (("time", 2 ** 32 - 1), ("pad", 65535), ("qtot", 65535), ("qmax", 65535), ("sigpad", 255), ("sigtime", 255), ("flags", 255)):
+        un[f][:5] = v
+    extra = np.zeros(3000, CLUSTER_DTYPE)
+    extra["sector"], extra["row"] = rng.integers(0, 36, 3000), rng.integers(0, 152, 3000)
+    extra["time"] = rng.integers(0, 1000, 3000)
+    _assert_unattached_encoding_equals_oracle(geo, np.concatenate((un, extra)))
+    # (c) nothing at all, and exactly one tile
+    _assert_unattached_encoding_equals_oracle(geo, np.zeros(0, CLUSTER_DTYPE))
+    one = np.zeros(2048, CLUSTER_DTYPE)
+    one["time"] = rng.permutation(2048)
+    _assert_unattached_encoding_equals_oracle(geo, one)
+    # a cluster without an output bin is reported
+    from paper_2411_02206_b200 import tmd as T
+    bad = np.zeros(10, CLUSTER_DTYPE)
+    bad["row"][3] = 200
+    with pytest.raises(T.TmdError) as e:
+        _gpu_encode_unattached(geo, bad)
+    assert e.value.status == T.TMD_ERR_CORRUPT

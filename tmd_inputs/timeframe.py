@@ -36,6 +36,7 @@ class Truth:
     trk_qptf: torch.Tensor   # float32 [n_tracks]
     att: torch.Tensor        # int32 [n_attached, 4] = 16-byte cluster records (layout.CLUSTER_DTYPE)
     leg: torch.Tensor        # uint8 [n_attached]
+    un: torch.Tensor | None = None   # int32 [n_unattached, 4] unattached clusters, any order (set by whoever draws them)
 
     @property
     def n_tracks(self) -> int:
