@@ -82,8 +82,6 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att, int n_sm) {
   w.o_rank16 = take((size_t)n_att * 2);
   w.o_inter = take((size_t)n_att * 8);
   w.o_table = take((size_t)TMD_MAX_BATCH * sizeof(FrameArgs));   // the frame table of a batch lives in frame 0's workspace
-  w.n_sort_words = ((n_tracks + SORT_WINDOW - 1) / SORT_WINDOW) * LEN_BINS;     // key histograms of the track sort (A2)
-  w.o_sort_hist = take((size_t)w.n_sort_words * 4);
   w.total = o;
   return w;
 }
@@ -217,10 +215,8 @@ int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t 
     TMD_LAUNCH("scan_tile_sums", k_scan_tile_sums<BATCH><<<dim3(1, nf), 1024, 0, st>>>(F0, table));
     TMD_LAUNCH("track_offsets", k_track_offsets<BATCH><<<dim3(mx.n_tiles, nf), SCAN_THREADS, 0, st>>>(F0, table));
     // A2: load-balance order (counting sort by cluster count, longest first, inside windows of consecutive tracks)
-    const uint32_t sort_blocks = (mx.n_tracks + SORT_BLOCK_TRACKS - 1) / SORT_BLOCK_TRACKS, sort_windows = (mx.n_tracks + SORT_WINDOW - 1) / SORT_WINDOW;
-    TMD_LAUNCH("sort_count", k_sort_count<BATCH><<<dim3(sort_blocks, nf), SORT_THREADS, 0, st>>>(F0, table));
-    TMD_LAUNCH("sort_scan", k_sort_scan<BATCH><<<dim3(sort_windows, nf), SORT_THREADS, 0, st>>>(F0, table));
-    TMD_LAUNCH("sort_place", k_sort_place<BATCH><<<dim3(sort_blocks, nf), SORT_THREADS, 0, st>>>(F0, table));
+    TMD_LAUNCH("len_sort_window",
+               k_len_sort_window<BATCH><<<dim3((mx.n_tracks + SORT_WINDOW - 1) / SORT_WINDOW, nf), SORT_THREADS, 0, st>>>(F0, table));
     // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
     const dim3 dg((mx.n_tracks + DECODE_THREADS - 1) / DECODE_THREADS, nf);
     if (mx.any_probe) TMD_LAUNCH("track_decode", k_track_decode<true, BATCH><<<dg, DECODE_THREADS, ctx->decode_smem, st>>>(G, F0, table));

@@ -68,10 +68,6 @@ __global__ void __launch_bounds__(1024) k_scan_tile_sums(const __grid_constant__
   uint32_t* __restrict__ tile_sum = F.at<uint32_t>(F.W.o_tile_sum);
   const uint32_t n_tiles = F.W.n_tiles;
   if (n_tiles == 0) return;
-  {  // the key histograms of the track sort (tmd_sort.cuh) start from zero
-    uint32_t* __restrict__ sh = F.at<uint32_t>(F.W.o_sort_hist);
-    for (uint32_t i = threadIdx.x; i < F.W.n_sort_words; i += blockDim.x) sh[i] = 0;
-  }
   uint32_t carry = 0;
   for (uint32_t base = 0; base < n_tiles; base += blockDim.x) {
     uint32_t i = base + threadIdx.x;
