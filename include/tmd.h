@@ -259,6 +259,35 @@ int tmd_encode_unattached_workspace_bytes(const tmd_ctx* ctx, uint64_t n_unattac
 int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster* un, tmd_compressed* out, void* workspace,
                           size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * Entropy stage in front of the decoder.  PAPER.md L20: the compressed time frames are written with
+ * "lossless ANS"; L49: "TPC Entropy Decoding" is the step right before track-model decoding; L68: the decoder's input is
+ * what "the entropy decoding" produces.  The paper gives no format; "TMDZ" is this build's own: every array
+ * of tmd_compressed is split into byte planes, each plane range-ANS coded (12-bit static table per plane, 32-bit state,
+ * 16-bit renormalisation) in blocks of 8192 symbols by 32 interleaved coders.
+ *
+ * tmd_entropy_bound:       upper bound of the container size for these counts.
+ * tmd_entropy_encode_host: HOST arrays in (`in`: host pointers), TMDZ container out (`blob`, HOST, capacity >= the bound).
+ *                          Runs on the calling host thread (the paper's rANS encoding is a CPU step of the synchronous
+ *                          phase, L40).
+ * tmd_entropy_sizes:       counts stored in a container's header (`head` = at least its first 64 bytes, HOST).
+ * tmd_entropy_decode:      decodes a container resident in DEVICE memory (`d_blob`, 16-byte aligned) into the DEVICE arrays
+ *                          `out` points to (caller-allocated with the counts of tmd_entropy_sizes, 16-byte aligned; out's
+ *                          n_tracks / n_attached / n_unattached must equal the header's).  `head` = HOST copy of the
+ *                          container's first 64 + 32 * 43 bytes (header + plane directory; the caller read the container
+ *                          from storage through host memory anyway).  Only enqueues one kernel on `cuda_stream`; one CTA
+ *                          decodes eight blocks (one per warp) and assembles 64 KiB of one array.  `d_err4` = 4 bytes of
+ *                          DEVICE memory that are non-zero afterwards if a table does not sum to 4096 or a block is too
+ *                          short (corrupt container; the output is then unspecified but nothing is written out of bounds).
+ *                          The arrays can be handed to tmd_decode on the same stream right away.
+ */
+int tmd_entropy_bound(uint32_t n_tracks, uint64_t n_attached, uint64_t n_unattached, uint32_t n_bins, size_t* out_bytes);
+int tmd_entropy_encode_host(const tmd_compressed* in, uint32_t n_bins, void* blob, size_t capacity, size_t* out_bytes);
+int tmd_entropy_sizes(const void* head, size_t head_bytes, uint32_t* n_tracks, uint64_t* n_attached, uint64_t* n_unattached,
+                      uint32_t* n_bins, size_t* blob_bytes);
+int tmd_entropy_decode(const void* head, size_t head_bytes, const void* d_blob, size_t blob_bytes, tmd_compressed* out, void* d_err4,
+                       void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -87,6 +87,12 @@ def lib() -> C.CDLL:
         L.tmd_encode_unattached_workspace_bytes.restype = C.c_int
         L.tmd_encode_unattached.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.POINTER(tmd_compressed), C.c_void_p, C.c_size_t, C.c_void_p]
         L.tmd_encode_unattached.restype = C.c_int
+        L.tmd_entropy_bound.argtypes = [C.c_uint32, C.c_uint64, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
+        L.tmd_entropy_encode_host.argtypes = [C.POINTER(tmd_compressed), C.c_uint32, C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.tmd_entropy_sizes.argtypes = [C.c_void_p, C.c_size_t, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), C.POINTER(C.c_size_t)]
+        L.tmd_entropy_decode.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p, C.c_size_t, C.POINTER(tmd_compressed), C.c_void_p, C.c_void_p]
+        for f in (L.tmd_entropy_bound, L.tmd_entropy_encode_host, L.tmd_entropy_sizes, L.tmd_entropy_decode):
+            f.restype = C.c_int
         L.tmd_selftest_ieee.argtypes = [C.c_uint32, C.POINTER(C.c_uint64)]
         L.tmd_selftest_ieee.restype = C.c_int
         L.tmd_decode_host_async.restype = C.c_int
@@ -245,3 +251,35 @@ def tmd_encode_unattached(ctx: int, un, out_arrays: dict, workspace, stream: int
             setattr(c, k, _ptr(out_arrays[k]))
     ws_bytes = int(workspace.numel() * workspace.element_size())
     _check(lib().tmd_encode_unattached(ctx, n, _ptr(un), C.byref(c), _ptr(workspace), ws_bytes, stream))
+
+
+ENTROPY_HEAD_BYTES = 64 + 32 * 43
+
+
+def tmd_entropy_bound(n_tracks: int, n_attached: int, n_unattached: int, n_bins: int) -> int:
+    out = C.c_size_t()
+    _check(lib().tmd_entropy_bound(n_tracks, n_attached, n_unattached, n_bins, C.byref(out)))
+    return out.value
+
+
+def tmd_entropy_encode_host(host_arrays: dict, n_bins: int) -> np.ndarray:
+    """Compressed SoA (HOST numpy arrays / CPU tensors) -> TMDZ container (numpy uint8 array), encoded on the host."""
+    comp = make_compressed(host_arrays)
+    cap = tmd_entropy_bound(comp.n_tracks, comp.n_attached, comp.n_unattached, n_bins)
+    blob = np.empty(cap, np.uint8)
+    n = C.c_size_t()
+    _check(lib().tmd_entropy_encode_host(C.byref(comp), n_bins, blob.ctypes.data, cap, C.byref(n)))
+    return blob[: n.value].copy()
+
+
+def tmd_entropy_sizes(head: np.ndarray) -> tuple[int, int, int, int, int]:
+    """(n_tracks, n_attached, n_unattached, n_bins, container bytes) from a container's first bytes (HOST)."""
+    a, b, c, d, e = C.c_uint32(), C.c_uint64(), C.c_uint64(), C.c_uint32(), C.c_size_t()
+    _check(lib().tmd_entropy_sizes(head.ctypes.data, head.size, C.byref(a), C.byref(b), C.byref(c), C.byref(d), C.byref(e)))
+    return a.value, b.value, c.value, d.value, e.value
+
+
+def tmd_entropy_decode(head: np.ndarray, d_blob, out_arrays: dict, d_err, stream: int = 0) -> None:
+    """Enqueue the decode of the TMDZ container `d_blob` (DEVICE uint8 tensor) into the DEVICE arrays of `out_arrays`."""
+    comp = make_compressed(out_arrays)
+    _check(lib().tmd_entropy_decode(head.ctypes.data, head.size, _ptr(d_blob), int(d_blob.numel()), C.byref(comp), _ptr(d_err), stream))

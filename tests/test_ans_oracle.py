@@ -151,3 +151,23 @@ def test_truncated_block_is_reported():
     blk = A.encode_block(sym, freq)
     with pytest.raises(RuntimeError):
         A.decode_block(blk[: len(blk) // 2], 4000, freq)
+
+
+# ------------------------------------------------------------------------------------------------ the library's host encoder
+def test_library_host_encoder_writes_containers_the_oracle_decodes(geo2, geo36):
+    # two independent encoders (oracle/tmd_ans.py and the library's tmd_entropy_encode_host, which share no code) must both
+    # write valid TMDZ: the oracle decoder restores the input from the library's container.  Runs without a GPU.
+    from paper_2411_02206_b200 import tmd as T
+    ev = ph.generate_event(ph.config0(), geo2)
+    for comp, n_bins in ((O.encode(geo2, 0.5, ev.trk_ncl, ev.trk_qptf, ev.att, ev.leg, ev.un), geo2.n_bins),
+                         (random_compressed(geo36, 200, 3000, 6), geo36.n_bins),
+                         (random_compressed(geo36, 0, 0, 7), geo36.n_bins)):
+        arrays = {k: np.ascontiguousarray(getattr(comp, k)) for k in COMPRESSED_FIELDS}
+        blob = T.tmd_entropy_encode_host(arrays, n_bins)
+        assert T.tmd_entropy_sizes(blob[:64])[:4] == (comp.n_tracks, comp.n_attached, comp.n_unattached, n_bins)
+        back = A.decode_container(blob)
+        for k in COMPRESSED_FIELDS:
+            assert np.array_equal(getattr(back, k), getattr(comp, k)), k
+        assert len(blob) <= T.tmd_entropy_bound(comp.n_tracks, comp.n_attached, comp.n_unattached, n_bins)
+        # the two encoders agree on the size within the freedom of the table quantisation
+        assert abs(len(blob) - len(A.encode_container(comp))) <= 0.01 * len(blob) + 64

@@ -400,3 +400,81 @@ def test_gpu_unattached_encoder_ties_skew_and_empty():
     with pytest.raises(T.TmdError) as e:
         _gpu_encode_unattached(geo, bad)
     assert e.value.status == T.TMD_ERR_CORRUPT
+
+
+# ------------------------------------------------------------------------------------------------ entropy stage (rANS) in front
+def _gpu_entropy_decode(blob: np.ndarray):
+    """tmd_entropy_decode of a TMDZ container -> (dict of device tensors, error word)."""
+    import torch
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    n_trk, n_att, n_un, n_bins, total = T.tmd_entropy_sizes(blob[:64])
+    assert total == blob.size
+    lens = {"n_tracks": n_trk, "n_attached": n_att, "n_residuals": n_att - n_trk, "n_unattached": n_un, "n_bins": n_bins}
+    tdt = {"<u2": torch.int16, "i1": torch.int8, "u1": torch.uint8, "<u4": torch.int32}
+    out = {k: torch.full((lens[w],), -86, dtype=tdt[dt], device="cuda") for k, (dt, w) in COMPRESSED_FIELDS.items()}
+    d_blob = torch.from_numpy(blob).cuda()
+    d_err = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T.tmd_entropy_decode(blob[:T.ENTROPY_HEAD_BYTES], d_blob, out, d_err, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out, int(d_err.item())
+
+
+def _assert_arrays_equal(out: dict, comp):
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    for k, (dt, _) in COMPRESSED_FIELDS.items():
+        got = out[k].cpu().numpy().view(np.dtype(dt))
+        assert np.array_equal(got, getattr(comp, k)), f"{k}: " + first_mismatch(got, getattr(comp, k))
+
+
+def test_entropy_decode_matches_oracle_and_feeds_the_decoder(phys_case):
+    # PAPER.md L49 / L68: entropy decoding, then track-model decoding.  The container is written by the ORACLE encoder; the GPU
+    # rANS decoder must restore every array of the compressed SoA bit for bit, and tmd_decode on those arrays (never leaving
+    # the device) must give the oracle decoder's clusters.
+    import torch
+    from oracle import tmd_ans as ANS
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs.layout import CLUSTER_DTYPE
+    name, geo, ev, comp = phys_case
+    blob = ANS.encode_container(comp)
+    out, err = _gpu_entropy_decode(blob)
+    assert err == 0
+    _assert_arrays_equal(out, comp)
+    if name in ("c0", "c2_like"):
+        ctx = T.tmd_create(geo, BZ)
+        try:
+            n = comp.n_attached + comp.n_unattached
+            d_cl = torch.empty(n * 16, dtype=torch.uint8, device="cuda")
+            d_bo = torch.empty(geo.n_bins + 1, dtype=torch.int32, device="cuda")
+            ws = torch.empty(T.tmd_workspace_bytes(ctx, comp.n_tracks, comp.n_attached, comp.n_unattached), dtype=torch.uint8, device="cuda")
+            T.tmd_decode(ctx, T.make_compressed(out), T.make_output(d_cl, d_bo, ws), 0, torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            want = O.decode(geo, BZ, comp)
+            assert np.array_equal(d_bo.cpu().numpy().view(np.uint32), want[1])
+            assert d_cl.cpu().numpy().view(CLUSTER_DTYPE).tobytes() == want[0].tobytes()
+        finally:
+            T.tmd_destroy(ctx)
+
+
+def test_entropy_decode_edge_cases_and_library_encoder():
+    from oracle import tmd_ans as ANS
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs.layout import COMPRESSED_FIELDS
+    geo = build_geometry(36)
+    cases = [random_compressed(geo, 3000, 40_000, 101, max_ncl=120),          # several 64 KiB chunks per array, ragged tails
+             random_compressed(geo, 1, 0, 102), random_compressed(geo, 0, 7, 103), Compressed.empty(0, 0, 0, geo.n_bins),
+             degenerate_same_bin(geo, np.full(400, 300, np.uint16), 104, n_un=50_001)]   # planes with one symbol only
+    for i, c in enumerate(cases):
+        for blob in (ANS.encode_container(c), T.tmd_entropy_encode_host({k: np.ascontiguousarray(getattr(c, k)) for k in COMPRESSED_FIELDS}, geo.n_bins)):
+            out, err = _gpu_entropy_decode(blob)
+            assert err == 0, i
+            _assert_arrays_equal(out, c)
+    # corrupt containers are reported, not followed out of bounds: a table that does not sum to 4096, a block table of garbage
+    c = cases[0]
+    blob = ANS.encode_container(c)
+    rec = blob[64:96]
+    t_off, b_off = int(rec[16:24].view(np.uint64)[0]), int(rec[24:32].view(np.uint64)[0])
+    bad = blob.copy(); bad[t_off:t_off + 2].view(np.uint16)[0] += 1
+    assert _gpu_entropy_decode(bad)[1] & 1
+    bad = blob.copy(); bad[b_off:b_off + 8].view(np.uint32)[:] = (0xFFFFFF00, 5)
+    assert _gpu_entropy_decode(bad)[1] & 4
