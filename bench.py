@@ -54,7 +54,7 @@ def kernel_algorithmic_bytes(n_trk: int, n_att: int, n_un: int, n_bins: int) -> 
 
 
 # ------------------------------------------------------------------------------------------------ workload on the device
-def build_workload(name: str, device, seed_offset: int = 0, keep_truth: bool = False):
+def build_workload(name: str, device, seed_offset: int = 0, keep_truth: bool = False, scale: float = 1.0):
     """Synthetic time frame `name` (tmd_inputs.timeframe.WORKLOADS) as device tensors of the compressed SoA: cluster truth
     (helix tracks + unattached clusters) -> the library's own encoder (tmd_encode_attached + tmd_encode_unattached), itself
     checked byte for byte against the oracle encoder in the -m gpu tests (bench.py may not run the oracle here)."""
@@ -66,6 +66,8 @@ def build_workload(name: str, device, seed_offset: int = 0, keep_truth: bool = F
     mk, n_un, single = tf.WORKLOADS[name]
     cfg = mk()
     cfg.seed += 1000 * seed_offset
+    if scale != 1.0:                                        # a fraction of the frame, same recipe (entropy-stage measurement)
+        cfg.n_tracks, n_un = max(1, int(cfg.n_tracks * scale)), int(n_un * scale)
     truth = tf.generate_truth(cfg, geo, device, batch=2_000_000)
     n_trk, n_att = truth.n_tracks, truth.n_attached
     arrays = {"trk_ncl": truth.trk_ncl}
@@ -402,6 +404,42 @@ def batch_workload(T, device, n_frames: int, steps: int, peak: float) -> dict | 
             "l2": "each frame is L2-sized; 64 frames = 3 GB of traffic per step, no flush"}
 
 
+def entropy_workload(T, device, steps: int, peak: float) -> dict | None:
+    """the entropy stage in front (PAPER.md L49 'TPC Entropy Decoding').  One eighth of a c2 frame is
+    written as a TMDZ container by the library's HOST encoder (one core, outside any timed region), copied to the device,
+    and the GPU rANS decode into the compressed SoA is timed alone and chained with tmd_decode on the same stream."""
+    import torch
+    if not hasattr(T, "tmd_entropy_decode"):
+        return None
+    geo, arrays = build_workload("c2", device, scale=0.125)
+    host = {k: v.cpu() for k, v in arrays.items()}
+    t0 = time.perf_counter()
+    blob = T.tmd_entropy_encode_host(host, geo.n_bins)
+    enc_s = time.perf_counter() - t0
+    raw = sum(v.numel() * v.element_size() for v in arrays.values())
+    d_blob = torch.from_numpy(blob).to(device)
+    d_err = torch.zeros(1, dtype=torch.int32, device=device)
+    out = {k: torch.empty_like(v) for k, v in arrays.items()}
+    head = blob[:T.ENTROPY_HEAD_BYTES]
+    stream = torch.cuda.current_stream().cuda_stream
+    ms_z = timed_steps(lambda: T.tmd_entropy_decode(head, d_blob, out, d_err, stream), steps, 3, torch.cuda.synchronize)
+    same = all(torch.equal(out[k], arrays[k]) for k in arrays) and int(d_err.item()) == 0
+    ctx = T.tmd_create(geo, BZ)
+    fr = Frame(T, ctx, geo, out, device)
+
+    def chain():
+        T.tmd_entropy_decode(head, d_blob, out, d_err, stream)
+        T.tmd_decode(ctx, fr.comp, fr.out, 0, stream)
+    ms_c = timed_steps(chain, steps, 3, torch.cuda.synchronize)
+    T.tmd_destroy(ctx)
+    sz, sc = stats(ms_z), stats(ms_c)
+    return {"workload": "one eighth of c2", "n_attached": fr.n_att, "n_unattached": fr.n_un, "raw_bytes": raw, "container_bytes": int(blob.size),
+            "compression": raw / blob.size, "restores_the_arrays": bool(same), "entropy_decode_ms": sz["mean"], "entropy_decode_ms_min": sz["min"],
+            "entropy_decode_out_gbs": raw / (sz["mean"] * 1e-3) / 1e9, "entropy_decode_frac_of_hbm_peak": (raw + blob.size) / (sz["mean"] * 1e-3) / 1e9 / peak,
+            "chain_ms": sc["mean"], "chain_clusters_per_s": fr.n_cl / (sc["mean"] * 1e-3), "host_encode_s": enc_s,
+            "l2": "container (%.0f MB) + arrays (%.0f MB): partly L2-resident (flag)" % (blob.size / 1e6, raw / 1e6)}
+
+
 def ncu_profile_numbers(kernel: str, workload: str):
     """(dram bytes per launch, warp instructions per launch, source file) of `kernel` from the committed ncu summary
     (profiles/traffic.txt: workload kernel dram_bytes warp_inst), else (None, None, None)."""
@@ -549,6 +587,10 @@ def run_ours(args) -> None:
             b = batch_workload(T, device, BATCH_FRAMES, min(args.steps, 10), peak)
             if b:
                 other[f"c1x{BATCH_FRAMES}"] = b
+            torch.cuda.empty_cache()
+            z = entropy_workload(T, device, min(args.steps, 10), peak)
+            if z:
+                other["entropy_stage"] = z
             line["other_workloads"] = other
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_tracks, device, value, not args.no_extras)

@@ -25,7 +25,7 @@ struct EncodeArgs {
 };
 
 __global__ void __launch_bounds__(128) k_encode_attached(DevGeo G, EncodeArgs A) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   RowGeo* rows = reinterpret_cast<RowGeo*>(smem_raw);
   for (uint32_t r = threadIdx.x; r < G.n_rows; r += blockDim.x) rows[r] = G.rows[r];
   __syncthreads();

@@ -105,7 +105,7 @@ __device__ __forceinline__ uint32_t un_bin_of_tile(const uint32_t* __restrict__ 
 
 // One block per tile: bitonic sort of up to UN_TILE records of ONE bin in shared memory (padding = records greater than any).
 __global__ void __launch_bounds__(UN_THREADS) k_un_sort_tiles(UnEncodeArgs A) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   uint4* s = reinterpret_cast<uint4*>(smem_raw);
   const uint32_t tile = blockIdx.x;
   if (tile >= A.tile_start[A.n_bins]) return;
@@ -141,7 +141,7 @@ __device__ __forceinline__ uint32_t un_merge_path(const uint4* a, uint32_t na, c
 
 // One block per output tile.  Pass `p` merges, inside every bin, runs of 2^p tiles pairwise (src -> dst).
 __global__ void __launch_bounds__(UN_THREADS) k_un_merge(UnEncodeArgs A, const uint4* __restrict__ src, uint4* __restrict__ dst, uint32_t p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   uint4* s = reinterpret_cast<uint4*>(smem_raw);
   __shared__ uint32_t s_split[2];
   const uint32_t tile = blockIdx.x;

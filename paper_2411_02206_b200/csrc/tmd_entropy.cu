@@ -25,6 +25,7 @@ constexpr uint32_t Z_L = 1u << 16;
 constexpr uint32_t Z_HEADER = 64, Z_PLANE = 32, Z_ARRAYS = 23, Z_PLANES = 43;
 constexpr int Z_THREADS = 256, Z_WARPS = 8;
 constexpr uint32_t Z_CHUNK_BYTES = Z_WARPS * Z_BLOCK;        // bytes of output one CTA assembles (65536)
+constexpr uint32_t Z_PARTS = 4, Z_PART = Z_BLOCK / Z_PARTS;   // a warp's block is decoded and written out in parts of 2048 symbols
 
 // widths (bytes per element) of the 23 arrays of tmd_compressed, in struct order
 __host__ __device__ inline uint32_t z_width(uint32_t a) {
@@ -50,8 +51,8 @@ static_assert(sizeof(ZArgs) < 3800, "kernel parameter space");
 // (wi mod w) into shared memory, then the CTA interleaves the planes into elements and writes them with coalesced stores.
 __global__ void __launch_bounds__(Z_THREADS) k_entropy_decode(const __grid_constant__ ZArgs Z, uint32_t* __restrict__ err) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  unsigned char* stage = smem_raw;                                            // [Z_WARPS][Z_BLOCK] decoded symbols
-  unsigned char* lut = smem_raw + Z_CHUNK_BYTES;                              // [w][4096] slot -> symbol
+  unsigned char* stage = smem_raw;                                            // [Z_WARPS][Z_PART] decoded symbols of the current part
+  unsigned char* lut = smem_raw + Z_WARPS * Z_PART;                           // [w][4096] slot -> symbol
   uint32_t* tab = reinterpret_cast<uint32_t*>(lut + 4 * Z_M);                  // [w][256] freq | cum << 16
   __shared__ uint32_t ws[33];
   // ---- which array, which chunk
@@ -70,25 +71,40 @@ __global__ void __launch_bounds__(Z_THREADS) k_entropy_decode(const __grid_const
     tab[j * 256 + tid] = f | (c << 16);                                        // c <= 4096 fits the upper half
     if (tid == 0 && total != Z_M) atomicOr(&err[0], 1u);
     __syncthreads();
-    for (uint32_t slot = tid; slot < Z_M; slot += Z_THREADS) {
-      // the largest symbol whose cumulative frequency is <= slot: symbols of frequency 0 share the cumulative value of their
-      // successor, so the largest index is the one that covers the slot
-      uint32_t lo = 0, hi = 255;
+    {
+      // slot -> symbol: the largest symbol whose cumulative frequency is <= slot (symbols of frequency 0 share the cumulative
+      // value of their successor, so the largest index is the one that covers the slot).  A thread fills 16 consecutive
+      // slots: one binary search for the first, then it walks up the cumulative table.
+      const uint32_t* t = tab + j * 256;
+      uint32_t slot = tid * (Z_M / Z_THREADS), lo = 0, hi = 255;
       while (lo < hi) {
         const uint32_t mid = (lo + hi + 1) >> 1;
-        if ((tab[j * 256 + mid] >> 16) <= slot) lo = mid; else hi = mid - 1;
+        if ((t[mid] >> 16) <= slot) lo = mid; else hi = mid - 1;
       }
-      lut[j * Z_M + slot] = (unsigned char)lo;
+      uint32_t packed[Z_M / Z_THREADS / 4];
+#pragma unroll
+      for (uint32_t k = 0; k < Z_M / Z_THREADS; ++k, ++slot) {
+        while (lo < 255 && (t[lo + 1] >> 16) <= slot) ++lo;
+        if ((k & 3u) == 0) packed[k >> 2] = 0;
+        packed[k >> 2] |= lo << (8 * (k & 3u));
+      }
+      uint4* dst4 = reinterpret_cast<uint4*>(lut + j * Z_M + tid * (Z_M / Z_THREADS));
+      static_assert(Z_M / Z_THREADS == 16, "one 16-byte store per thread");
+      *dst4 = make_uint4(packed[0], packed[1], packed[2], packed[3]);
     }
     __syncthreads();
   }
-  // ---- decode: one block per warp
+  // ---- decode: one block per warp, in Z_PARTS parts of Z_PART symbols; after each part the CTA interleaves the planes into
+  // elements and writes them out (a part-sized staging buffer keeps six CTAs resident per SM: the decode loop is a chain
+  // of dependent look-ups and shuffles, it needs many warps to hide its latency)
   const uint32_t j = wi % w, q = wi / w, per_plane = Z_WARPS / w;
   const uint64_t n_sym = A.n_elem;
   const uint64_t b = (uint64_t)chunk * per_plane + q;                           // block index inside the plane
   const uint64_t first = b * Z_BLOCK;
-  if (first < n_sym) {
-    const uint32_t n = (uint32_t)min((uint64_t)Z_BLOCK, n_sym - first);
+  const uint32_t n = first < n_sym ? (uint32_t)min((uint64_t)Z_BLOCK, n_sym - first) : 0u;   // symbols of this warp's block
+  uint32_t x = 0, used = 0, base = 0, w0 = 0, w1 = 0, max_words = 0;
+  const uint16_t* words = nullptr;
+  if (n) {
     const uint32_t* starts = reinterpret_cast<const uint32_t*>(Z.blob + Z.pl[A.first_plane + j].blocks_offset);
     uint32_t s0 = starts[b], s1 = starts[b + 1];
     if (s1 < s0 || s1 > Z.blob_bytes || s1 - s0 < 4 * Z_LANES) {               // corrupt block table: decode nothing from it
@@ -96,41 +112,79 @@ __global__ void __launch_bounds__(Z_THREADS) k_entropy_decode(const __grid_const
       s0 = 0; s1 = 4 * Z_LANES;
     }
     const unsigned char* blk = Z.blob + s0;
-    uint32_t x = reinterpret_cast<const uint32_t*>(blk)[lane];
-    const uint16_t* words = reinterpret_cast<const uint16_t*>(blk + 4 * Z_LANES);
-    const uint32_t max_words = s1 > s0 + 4 * Z_LANES ? (s1 - s0 - 4 * Z_LANES) / 2 : 0;
-    uint32_t used = 0;
-    const unsigned char* my_lut = lut + j * Z_M;
-    const uint32_t* my_tab = tab + j * 256;
-    unsigned char* dst = stage + wi * Z_BLOCK;
-    for (uint32_t k0 = 0; k0 < n; k0 += 32) {
+    x = reinterpret_cast<const uint32_t*>(blk)[lane];
+    words = reinterpret_cast<const uint16_t*>(blk + 4 * Z_LANES);
+    max_words = (s1 - s0 - 4 * Z_LANES) / 2;
+  }
+  // The words the warp will read next sit in two registers per lane (a 64-word window starting at `base`): a lane takes
+  // its word with a shuffle, and the window is refilled 32 words ahead of its use, so no global-memory latency is on the
+  // loop-carried path (state -> table look-ups -> ballot -> word).
+  auto load_words = [&](uint32_t at) -> uint32_t { return at < max_words ? (uint32_t)__ldg(words + at) : 0u; };
+  w0 = load_words(lane); w1 = load_words(32 + lane);
+  // shared-memory addresses of this warp's tables and staging row, computed once (the loop below is issue-bound)
+  const uint32_t lut_a = (uint32_t)__cvta_generic_to_shared(lut + j * Z_M), tab_a = (uint32_t)__cvta_generic_to_shared(tab + j * 256);
+  const uint32_t dst_a = (uint32_t)__cvta_generic_to_shared(stage + wi * Z_PART) + lane;
+  const uint32_t wshift = w == 4 ? 2 : (w == 2 ? 1 : 0);
+  const uint64_t total_bytes = n_sym * w;
+  for (uint32_t part = 0; part < Z_PARTS; ++part) {
+    const uint32_t k_lo = part * Z_PART, k_hi = min(n, k_lo + Z_PART);
+    for (uint32_t k0 = k_lo; k0 < k_hi; k0 += 32) {
       const bool active = k0 + lane < n;
-      const uint32_t slot = x & (Z_M - 1), s = my_lut[slot], fc = my_tab[s];
+      const uint32_t slot = x & (Z_M - 1);
+      uint32_t s, fc;
+      asm volatile("ld.shared.u8 %0, [%1];" : "=r"(s) : "r"(lut_a + slot));
+      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(fc) : "r"(tab_a + (s << 2)));
       uint32_t xn = (fc & 0xFFFFu) * (x >> Z_PROB_BITS) + slot - (fc >> 16);
       const bool need = active && xn < Z_L;
       const uint32_t mask = __ballot_sync(0xffffffffu, need);
-      if (need) {
-        const uint32_t at = used + __popc(mask & ((1u << lane) - 1u));
-        xn = (xn << 16) | (at < max_words ? (uint32_t)words[at] : 0u);
-      }
+      const uint32_t idx = used - base + __popc(mask & ((1u << lane) - 1u));          // 0 .. 63 inside the window
+      const uint32_t c0 = __shfl_sync(0xffffffffu, w0, idx & 31u), c1 = __shfl_sync(0xffffffffu, w1, idx & 31u);
+      if (need) xn = (xn << 16) | (idx < 32u ? c0 : c1);
       used += __popc(mask);
-      if (active) { x = xn; dst[k0 + lane] = (unsigned char)s; }
+      if (used - base >= 32u) {                                                      // warp-uniform
+        base += 32u;
+        w0 = w1;
+        w1 = load_words(base + 32u + lane);
+      }
+      if (active) {
+        x = xn;
+        asm volatile("st.shared.u8 [%0], %1;" ::"r"(dst_a + (k0 - k_lo)), "r"(s) : "memory");
+      }
     }
-    if (lane == 0 && used > max_words) atomicOr(&err[0], 2u);                  // a block shorter than its symbols need
+    __syncthreads();
+    // interleave the planes into elements.  The part holds, for every block q of the chunk, elements [q * 8192 + part * 2048,
+    // + 2048): byte jj of local element i of block q is stage[(q * w + jj) * Z_PART + i].
+    // 16 output bytes per thread and step: 16 / w consecutive elements, their bytes fetched with one vector load per plane
+    const uint32_t vec_per_q = (Z_PART * w) >> 4;                                     // 16-byte vectors of output per block and part
+    for (uint32_t t = tid; t < per_plane * vec_per_q; t += Z_THREADS) {
+      const uint32_t qq = t / vec_per_q, o = (t - qq * vec_per_q) << 4;               // byte offset inside the (block, part) piece
+      const uint64_t out_byte = (uint64_t)chunk * Z_CHUNK_BYTES + ((uint64_t)qq * Z_BLOCK + (uint64_t)part * Z_PART) * w + o;
+      if (out_byte >= total_bytes) continue;
+      const unsigned char* src = stage + (qq * w) * Z_PART + (o >> wshift);           // plane 0 of the first element of the vector
+      uint4 v;
+      if (w == 1) {
+        v = *reinterpret_cast<const uint4*>(src);
+      } else if (w == 2) {
+        const uint2 lo = *reinterpret_cast<const uint2*>(src), hi = *reinterpret_cast<const uint2*>(src + Z_PART);
+        v.x = __byte_perm(lo.x, hi.x, 0x5140); v.y = __byte_perm(lo.x, hi.x, 0x7362);
+        v.z = __byte_perm(lo.y, hi.y, 0x5140); v.w = __byte_perm(lo.y, hi.y, 0x7362);
+      } else {
+        const uint32_t p0 = *reinterpret_cast<const uint32_t*>(src), p1 = *reinterpret_cast<const uint32_t*>(src + Z_PART);
+        const uint32_t p2 = *reinterpret_cast<const uint32_t*>(src + 2 * Z_PART), p3 = *reinterpret_cast<const uint32_t*>(src + 3 * Z_PART);
+        const uint32_t a01 = __byte_perm(p0, p1, 0x5140), b01 = __byte_perm(p0, p1, 0x7362);   // (p0.b0 p1.b0 p0.b1 p1.b1), (.. b2 .. b3)
+        const uint32_t a23 = __byte_perm(p2, p3, 0x5140), b23 = __byte_perm(p2, p3, 0x7362);
+        v.x = __byte_perm(a01, a23, 0x5410); v.y = __byte_perm(a01, a23, 0x7632);
+        v.z = __byte_perm(b01, b23, 0x5410); v.w = __byte_perm(b01, b23, 0x7632);
+      }
+      if (out_byte + 16 <= total_bytes) *reinterpret_cast<uint4*>(A.out + out_byte) = v;
+      else {
+        const uint32_t vv[4] = {v.x, v.y, v.z, v.w};
+        for (uint32_t kb = 0; out_byte + kb < total_bytes; ++kb) A.out[out_byte + kb] = (unsigned char)(vv[kb >> 2] >> (8 * (kb & 3u)));
+      }
+    }
+    __syncthreads();
   }
-  __syncthreads();
-  // ---- interleave the planes into elements: output byte o of the chunk = byte (o mod w) of element (o / w)
-  const uint64_t out0 = (uint64_t)chunk * Z_CHUNK_BYTES, total_bytes = n_sym * w;
-  const uint32_t n_out = (uint32_t)min((uint64_t)Z_CHUNK_BYTES, total_bytes - out0);
-  const uint32_t wshift = w == 4 ? 2 : (w == 2 ? 1 : 0);
-  auto byte_at = [&](uint32_t o) -> uint32_t {
-    const uint32_t e = o >> wshift, jj = o & (w - 1);                          // element (inside the chunk), plane
-    return stage[((e / Z_BLOCK) * w + jj) * Z_BLOCK + (e % Z_BLOCK)];
-  };
-  uint32_t* out32 = reinterpret_cast<uint32_t*>(A.out + out0);                 // 16-byte aligned array, out0 multiple of 65536
-  for (uint32_t o = tid * 4; o + 4 <= n_out; o += Z_THREADS * 4)
-    out32[o >> 2] = byte_at(o) | (byte_at(o + 1) << 8) | (byte_at(o + 2) << 16) | (byte_at(o + 3) << 24);
-  if (tid < (n_out & 3u)) A.out[out0 + (n_out & ~3u) + tid] = (unsigned char)byte_at((n_out & ~3u) + tid);
+  if (n && lane == 0 && used > max_words) atomicOr(&err[0], 2u);               // a block shorter than its symbols need
 }
 
 // ---------------------------------------------------------------------------------------------------------------- host side
@@ -335,7 +389,7 @@ int tmd_entropy_decode(const void* head, size_t head_bytes, const void* d_blob, 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (cudaMemsetAsync(d_err4, 0, 4, st) != cudaSuccess) return TMD_ERR_CUDA;
   if (chunk == 0) return TMD_OK;
-  const size_t smem = Z_CHUNK_BYTES + 4 * (size_t)Z_M + 4 * 256 * 4;
+  const size_t smem = (size_t)Z_WARPS * Z_PART + 4 * (size_t)Z_M + 4 * 256 * 4;
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(k_entropy_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return TMD_ERR_CUDA;

@@ -84,7 +84,7 @@ __device__ __forceinline__ uint32_t warp_rank32(uint16_t* cnt, uint32_t b, uint3
 template <bool BATCH>
 __global__ void __launch_bounds__(WR_THREADS) k_rank(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
                                                      const FrameArgs* __restrict__ table) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const uint32_t lane = lane_id(), wib = threadIdx.x >> 5, n_bins = G.n_bins;
   const RankArgs A = rank_args(frame_of<BATCH>(F0, table, blockIdx.y), n_bins);
   const uint32_t cnt_bytes = wr_warp_smem(n_bins);

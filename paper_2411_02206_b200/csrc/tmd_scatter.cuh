@@ -71,22 +71,29 @@ __device__ __forceinline__ ScatterArgs scatter_args(const FrameArgs& F, uint32_t
 template <bool BATCH>
 __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
                                                            const FrameArgs* __restrict__ table) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
   if ((blockIdx.x >> SC_CLUSTER_SHIFT) >= F.W.n_chunks) return;     // uniform over the cluster: nobody is left waiting
   const ScatterArgs A = scatter_args(F, G.n_bins);
   uint4* recs = reinterpret_cast<uint4*>(smem_raw);                                   // this CTA's part of the sorted chunk
+  const uint32_t recs_addr = (uint32_t)__cvta_generic_to_shared(smem_raw);
   uint16_t* start = reinterpret_cast<uint16_t*>(smem_raw + (size_t)SC_MAX_PER_CTA * 16);  // [n_bins + 1] first slot of every bin
   cg::cluster_group cluster = cg::this_cluster();
   const uint32_t rank_in_cluster = cluster.block_rank();
   const uint32_t c = blockIdx.x >> SC_CLUSTER_SHIFT, tid = threadIdx.x, n_bins = G.n_bins;
   const uint32_t per_shift = A.chunk_shift - SC_CLUSTER_SHIFT, per_cta = 1u << per_shift;
-  cluster.barrier_arrive();                          // "this CTA is running": waited for just before the first remote store
-  // ---- start[bin]: the chunk's row of the table the rank kernel wrote (every CTA keeps a copy)
-  {
-    const uint4* src = reinterpret_cast<const uint4*>(A.start16 + (size_t)c * A.start_stride);
-    for (uint32_t i = tid; i < A.start_stride / 8; i += SC_THREADS) reinterpret_cast<uint4*>(start)[i] = __ldg(src + i);
+  // ---- arrival of the sorted records is tracked by a transaction barrier in every CTA: a remote store (st.async) completes
+  // 16 bytes on the DESTINATION's barrier, and a CTA waits only until the bytes of ITS part have landed -- no cluster-wide
+  // barrier with release semantics (MEMBAR.ALL.GPU + ERRBAR + the wait for the slowest CTA: 26 % of the stall samples).
+  __shared__ __align__(8) unsigned long long mbar;
+  const uint32_t mbar_addr = (uint32_t)__cvta_generic_to_shared(&mbar);
+  const uint32_t n_valid = __ldg(A.start16 + (size_t)c * A.start_stride + n_bins);      // records of the chunk that have a bin (used late)
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // "this CTA is running and its barrier exists": waited for just before the first remote store
+  asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");     // (the mbarrier_init fence above is the release it needs)
   // ---- this CTA's share of g: loads in flight before the cluster barrier
   const uint32_t g_base = (c << A.chunk_shift) + (rank_in_cluster << per_shift);
   bool first = true;
@@ -104,8 +111,14 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
       }
     }
     if (first) {
+      // start[bin]: the chunk's row of the table the rank kernel wrote (every CTA keeps a copy); requested AFTER the first
+      // batch of record loads so that its latency overlaps theirs
+      const uint4* src = reinterpret_cast<const uint4*>(A.start16 + (size_t)c * A.start_stride);
+      for (uint32_t i = tid; i < A.start_stride / 8; i += SC_THREADS) cp_async16(reinterpret_cast<uint4*>(start) + i, src + i, 16);
+      cp_async_commit();
+      cp_async_wait<0>();                            // (asynchronous copies: no registers held next to the record loads)
       __syncthreads();                               // start[] visible
-      cluster.barrier_wait();                        // every CTA of the cluster is running (they arrived before their loads)
+      asm volatile("barrier.cluster.wait.aligned;" ::: "memory");   // every CTA of the cluster is running (they arrived before their loads)
       first = false;
     }
 #pragma unroll
@@ -114,13 +127,27 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
       if (bin == BIN_INVALID) continue;              // no output bin (reading 20), or past the end
       const uint32_t sec = (bin * G.rows_magic) >> 24, row = bin - sec * G.n_rows;
       const uint32_t slot = (uint32_t)start[bin] + rk[k];
-      uint4* remote = cluster.map_shared_rank(recs, slot >> per_shift);
-      remote[slot & (per_cta - 1)] = pack_cluster(rec[k].x, rec[k].y & 0xFFFFu, qt[k], qm[k], sp[k], st[k], fl[k], row, sec);
+      const uint4 v = pack_cluster(rec[k].x, rec[k].y & 0xFFFFu, qt[k], qm[k], sp[k], st[k], fl[k], row, sec);
+      const uint32_t dst_cta = slot >> per_shift;
+      uint32_t r_addr, r_mbar;
+      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r_addr) : "r"(recs_addr + ((slot & (per_cta - 1)) << 4)), "r"(dst_cta));
+      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r_mbar) : "r"(mbar_addr), "r"(dst_cta));
+      asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(r_addr),
+                   "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"(r_mbar)
+                   : "memory");
     }
   }
-  cluster.sync();                                    // the sorted chunk is complete
+  // ---- wait until this CTA's part of the sorted chunk is complete (phase 0 of the transaction barrier).  The expected byte
+  // count is posted only now (the remote completions may come first: the barrier's pending count goes negative meanwhile)
+  const uint32_t my_first = rank_in_cluster << per_shift;
+  const uint32_t n_expected = n_valid > my_first ? min(n_valid - my_first, per_cta) : 0u;   // records that land here
+  if (tid == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(n_expected * 16u) : "memory");
+  if (n_expected) {
+    uint32_t done = 0;
+    while (!done)
+      asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar_addr) : "memory");
+  }
   // ---- this CTA's part of the sorted chunk to its canonical positions
-  const uint32_t n_valid = start[n_bins];
   const uint32_t* __restrict__ rel_row = A.rel + (size_t)c * n_bins;
   uint4* __restrict__ out = A.clusters;
   for (uint32_t i0 = 0; i0 < per_cta; i0 += SC_THREADS * SC_UNROLL) {
