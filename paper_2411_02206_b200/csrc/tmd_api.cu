@@ -359,11 +359,11 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   const uint32_t n_bins_c = g->n_sectors_out * g->n_rows;
   ctx->rank_smem = (size_t)WR_WARPS * wr_warp_smem(n_bins_c);
   ctx->scatter_smem = sc_smem_bytes(n_bins_c);
-  ctx->decode_smem = DECODE_STAGE_BYTES + sizeof(RowGeo) * g->n_rows;
+  ctx->decode_smem = decode_smem_bytes(g->n_rows);
   // The dynamic shared-memory limit is a per-function, process-wide attribute: always set it to the maximum any geometry
   // can need (MAX_BINS bins, 255 rows), so that contexts of different geometries never lower it for one another.
   const size_t rank_max = (size_t)WR_WARPS * wr_warp_smem(MAX_BINS), scatter_max = sc_smem_bytes(MAX_BINS);
-  const size_t decode_max = DECODE_STAGE_BYTES + sizeof(RowGeo) * 255;
+  const size_t decode_max = decode_smem_bytes(255);
   if (e == cudaSuccess) e = allow_smem(k_rank<false>, rank_max);
   if (e == cudaSuccess) e = allow_smem(k_rank<true>, rank_max);
   if (e == cudaSuccess) e = allow_smem(k_scatter<false>, scatter_max);

@@ -99,14 +99,14 @@ __global__ void __launch_bounds__(WR_THREADS) k_rank(const __grid_constant__ Dev
 #pragma unroll
     for (int k = 0; k < WR_DEPTH; ++k) {
       const uint32_t g = g0 + k * 32 + lane;
-      cur[k] = g < g1 ? __ldg(&A.inter[g].y) : 0xFFFFFFFFu;         // raw word: the bin is taken at the use, not here
+      cur[k] = g < g1 ? __ldcg(&A.inter[g].y) : 0xFFFFFFFFu;         // raw word: the bin is taken at the use, not here
     }
     for (uint32_t gb = g0; gb < g1; gb += WR_DEPTH * 32) {
       uint32_t runs[WR_DEPTH];
       if (gb + 2 * WR_DEPTH * 32 <= g1) {                           // this batch and the next lie inside the chunk: no guards
         const uint32_t* src = &A.inter[gb + WR_DEPTH * 32 + lane].y;
 #pragma unroll
-        for (int k = 0; k < WR_DEPTH; ++k) nxt[k] = __ldg(src + k * 64);   // 32 records of 8 bytes further on
+        for (int k = 0; k < WR_DEPTH; ++k) nxt[k] = __ldcg(src + k * 64);   // 32 records of 8 bytes further on
 #pragma unroll
         for (int k = 0; k < WR_DEPTH; ++k) runs[k] = warp_runs(cur[k] >> 16, lane);
         uint16_t* dst = A.rank16 + gb + lane;
@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(WR_THREADS) k_rank(const __grid_constant__ Dev
 #pragma unroll
         for (int k = 0; k < WR_DEPTH; ++k) {
           const uint32_t g = gb + (WR_DEPTH + k) * 32 + lane;
-          nxt[k] = g < g1 ? __ldg(&A.inter[g].y) : 0xFFFFFFFFu;     // no use of the value before the next batch
+          nxt[k] = g < g1 ? __ldcg(&A.inter[g].y) : 0xFFFFFFFFu;     // no use of the value before the next batch
         }
 #pragma unroll
         for (int k = 0; k < WR_DEPTH; ++k) runs[k] = warp_runs(cur[k] >> 16, lane);
