@@ -72,7 +72,8 @@ Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att, int n_sm) {
   w.o_err = take(ERR_WORDS * 4);
   w.o_tile_sum = take(((size_t)w.n_tiles + 1) * 4);
   w.o_off = take(((size_t)n_tracks + 1) * 4);
-  w.o_perm = take((size_t)n_tracks * 4);
+  w.o_hdr = take((size_t)n_tracks * 16);      // per-track header records in load-balance order (A2), see tmd_sort.cuh
+  w.o_hdr2 = take((size_t)n_tracks * 4);
   w.o_att_cnt = take((size_t)n_bins * 4);
   w.o_u_start = take(((size_t)n_bins + 1) * 4);
   w.o_gsum = take((size_t)w.n_groups * n_bins * 4);

@@ -41,7 +41,7 @@ enum { ERR_TRACK_FIELD = 0, ERR_SECTOR_OUT = 1, ERR_NCL_SUM_LO = 2, ERR_NCL_SUM_
 // counts.  A pure function of (n_bins, n_tracks, n_attached, SM count): tmd_workspace_bytes and tmd_decode agree.
 struct Workspace {
   uint32_t n_tiles, n_chunks, n_groups, chunk_shift;
-  size_t o_err, o_tile_sum, o_off, o_perm, o_att_cnt, o_u_start, o_gsum, o_hist, o_start16, o_rel, o_rank16, o_inter, o_table, total;
+  size_t o_err, o_tile_sum, o_off, o_hdr, o_hdr2, o_att_cnt, o_u_start, o_gsum, o_hist, o_start16, o_rel, o_rank16, o_inter, o_table, total;
 };
 
 // Everything the kernels need to know about ONE time frame.  tmd_decode passes it by value (kernel parameter space);

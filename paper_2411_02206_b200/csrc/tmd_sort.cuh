@@ -5,6 +5,11 @@
 // tracks spans a few MB of each stream), which keeps the working set of pages small.
 // The permutation only decides which thread decodes which track: the output order is fixed by C5 and does not depend
 // on it (ties inside a length class are placed in arbitrary order).  Integer only.
+// The kernel does not write the permutation itself but, in that order, a HEADER RECORD per track with everything the decode
+// kernel needs to start it: hdr[p] = {off[t], t, trk_time0[t], trk_ncl[t] | trk_pad0[t] << 16} and
+// hdr2[p] = trk_sec0[t] | trk_row0[t] << 8 | (uint8)trk_qpt[t] << 16.  A decode thread then starts with two coalesced loads
+// instead of three dependent round trips (perm -> off / sector / row -> pad / time / q/pT, each a scattered sector):
+// timestamps showed 10.6 us from block start to the first step of a 129 us block at c3.
 #pragma once
 
 #include "tmd_common.cuh"
@@ -30,18 +35,21 @@ __global__ void __launch_bounds__(SORT_THREADS) k_len_sort_window(const __grid_c
   const uint32_t n_tracks = F.in.n_tracks;
   if (blockIdx.x * SORT_WINDOW >= n_tracks) return;
   const uint16_t* __restrict__ trk_ncl = F.in.trk_ncl;
-  uint32_t* __restrict__ perm = F.at<uint32_t>(F.W.o_perm);
+  uint4* __restrict__ hdr = F.at<uint4>(F.W.o_hdr);
+  uint32_t* __restrict__ hdr2 = F.at<uint32_t>(F.W.o_hdr2);
+  const uint32_t* __restrict__ off = F.at<uint32_t>(F.W.o_off);
   h[threadIdx.x] = 0;
   h[threadIdx.x + SORT_THREADS] = 0;
   __syncthreads();
   const uint32_t base = blockIdx.x * SORT_WINDOW;
-  uint32_t cls[SORT_ITEMS], loc[SORT_ITEMS];
+  uint32_t cls[SORT_ITEMS], loc[SORT_ITEMS], ncl[SORT_ITEMS];
 #pragma unroll
   for (int k = 0; k < SORT_ITEMS; ++k) {
     const uint32_t t = base + k * SORT_THREADS + threadIdx.x;
-    cls[k] = 0; loc[k] = 0;
+    cls[k] = 0; loc[k] = 0; ncl[k] = 0;
     if (t < n_tracks) {
-      cls[k] = len_class(trk_ncl[t]);
+      ncl[k] = trk_ncl[t];
+      cls[k] = len_class(ncl[k]);
       loc[k] = atomicAdd(&h[cls[k]], 1u);
     }
   }
@@ -59,7 +67,11 @@ __global__ void __launch_bounds__(SORT_THREADS) k_len_sort_window(const __grid_c
 #pragma unroll
   for (int k = 0; k < SORT_ITEMS; ++k) {
     const uint32_t t = base + k * SORT_THREADS + threadIdx.x;
-    if (t < n_tracks) perm[base + h[cls[k]] + loc[k]] = t;
+    if (t < n_tracks) {
+      const uint32_t p = base + h[cls[k]] + loc[k];
+      hdr[p] = make_uint4(off[t], t, F.in.trk_time0[t], ncl[k] | ((uint32_t)F.in.trk_pad0[t] << 16));
+      hdr2[p] = (uint32_t)F.in.trk_sec0[t] | ((uint32_t)F.in.trk_row0[t] << 8) | ((uint32_t)(uint8_t)F.in.trk_qpt[t] << 16);
+    }
   }
 }
 
