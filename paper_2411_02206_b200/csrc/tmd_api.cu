@@ -1,5 +1,6 @@
 // tmd_api.cu -- the C ABI of libtmd.so (include/tmd.h): context, workspace layout, kernel sequencing.
 // Every step of the path runs in the kernels of this directory; the host code only checks arguments and enqueues.
+#include <algorithm>
 #include <new>
 #include <stdlib.h>
 #include <string.h>
@@ -22,7 +23,8 @@ struct tmd_ctx {
   int device;
   int n_sm;                    // cudaDevAttrMultiProcessorCount
   size_t smem_per_sm;          // cudaDevAttrMaxSharedMemoryPerMultiprocessor
-  size_t decode_smem, rank_smem, scatter_smem;
+  size_t smem_reserved;        // cudaDevAttrReservedSharedMemoryPerBlock
+  size_t decode_smem, decode_smem_max, rank_smem, scatter_smem;
   // Per-call state.  `launches` is the launch count of the last tmd_decode / tmd_decode_batch (the same for every call
   // with the same flags and emptiness, so concurrent calls store the same value).  The TMD_TIMING event pairs and the
   // host-pipeline slots are the only other state a call touches: calls with TMD_TIMING, and the tmd_decode_host* entry
@@ -202,7 +204,7 @@ struct Launcher {
 // The launch sequence of rows A1-A7 over `n_frames` frames.  BATCH = false: one frame, its FrameArgs
 // passed by value.  BATCH = true: the frames' FrameArgs are in device memory (`table`) and every grid has a frame
 // coordinate; `mx` holds the per-kernel maxima of the frames' grid extents.
-struct Extents { uint32_t n_tiles, n_tracks, n_chunks, n_groups; uint64_t n_unattached; bool any_probe; };
+struct Extents { uint32_t n_tiles, n_tracks, n_chunks, n_groups; uint64_t n_unattached; bool any_probe; uint32_t mean_len; };   // mean_len: attached clusters per track (all frames)
 
 template <bool BATCH>
 int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t n_frames, const Extents& mx, Launcher& L) {
@@ -219,9 +221,18 @@ int enqueue(tmd_ctx* ctx, const FrameArgs& F0, const FrameArgs* table, uint32_t 
     TMD_LAUNCH("len_sort_window",
                k_len_sort_window<BATCH><<<dim3((mx.n_tracks + SORT_WINDOW - 1) / SORT_WINDOW, nf), SORT_THREADS, 0, st>>>(F0, table));
     // A3 (walk) + A5: track-model decode -> intermediate records {T, P, bin} in g order
+    // Blocks per SM: registers allow DECODE_BLOCKS_PER_SM = 6; for long tracks 5 are faster (c3 2.39 -> 2.28 ms, 4: 2.30, 7: 2.52,
+    // 8: 2.62: every track in flight keeps five 128-byte lines alive in the L2 -- four streams and its output -- and 113 k tracks
+    // x 5 lines overflow it: sectors are evicted between the two cells that share them), for short tracks 6 (c4 1.24 vs 1.28 ms:
+    // more tracks start per unit of time).  The cap is set through the size of the dynamic shared memory.
     const dim3 dg((mx.n_tracks + DECODE_THREADS - 1) / DECODE_THREADS, nf);
-    if (mx.any_probe) TMD_LAUNCH("track_decode", k_track_decode<true, BATCH><<<dg, DECODE_THREADS, ctx->decode_smem, st>>>(G, F0, table));
-    else TMD_LAUNCH("track_decode", k_track_decode<false, BATCH><<<dg, DECODE_THREADS, ctx->decode_smem, st>>>(G, F0, table));
+    size_t dsm = ctx->decode_smem;
+    if (mx.mean_len >= DECODE_LONG_TRACKS) {
+      const size_t cap = ctx->smem_per_sm / DECODE_BLOCKS_PER_SM - ctx->smem_reserved + 128;   // DECODE_BLOCKS_PER_SM blocks of this size do not fit
+      if (cap > dsm && cap <= ctx->decode_smem_max) dsm = cap;
+    }
+    if (mx.any_probe) TMD_LAUNCH("track_decode", k_track_decode<true, BATCH><<<dg, DECODE_THREADS, dsm, st>>>(G, F0, table));
+    else TMD_LAUNCH("track_decode", k_track_decode<false, BATCH><<<dg, DECODE_THREADS, dsm, st>>>(G, F0, table));
     // A3 (count): per-chunk histogram + ranks; one warp per chunk, as many warps resident as shared memory allows
     uint32_t per_sm = (uint32_t)(ctx->smem_per_sm / (ctx->rank_smem + 1024));
     if (per_sm < 1) per_sm = 1;
@@ -357,6 +368,9 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, ctx->device);
   ctx->smem_per_sm = (size_t)smem_sm;
+  int smem_res = 0;
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_res, cudaDevAttrReservedSharedMemoryPerBlock, ctx->device);
+  ctx->smem_reserved = (size_t)smem_res;
   const uint32_t n_bins_c = g->n_sectors_out * g->n_rows;
   ctx->rank_smem = (size_t)WR_WARPS * wr_warp_smem(n_bins_c);
   ctx->scatter_smem = sc_smem_bytes(n_bins_c);
@@ -364,7 +378,9 @@ int tmd_create(const tmd_geometry* g, const tmd_field* f, tmd_ctx** out_ctx) {
   // The dynamic shared-memory limit is a per-function, process-wide attribute: always set it to the maximum any geometry
   // can need (MAX_BINS bins, 255 rows), so that contexts of different geometries never lower it for one another.
   const size_t rank_max = (size_t)WR_WARPS * wr_warp_smem(MAX_BINS), scatter_max = sc_smem_bytes(MAX_BINS);
-  const size_t decode_max = decode_smem_bytes(255);
+  // (the decode kernel may be launched with more than it needs: that is how its blocks per SM are capped, see enqueue)
+  const size_t decode_max = std::max(decode_smem_bytes(255), ctx->smem_per_sm / (DECODE_BLOCKS_PER_SM - 1) - ctx->smem_reserved);
+  ctx->decode_smem_max = decode_max;
   if (e == cudaSuccess) e = allow_smem(k_rank<false>, rank_max);
   if (e == cudaSuccess) e = allow_smem(k_rank<true>, rank_max);
   if (e == cudaSuccess) e = allow_smem(k_scatter<false>, scatter_max);
@@ -441,7 +457,8 @@ int tmd_decode(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t
     TMD_CUDA(cudaMemsetAsync(d_err, 0, ERR_WORDS * 4, st));
   }
   Launcher L{ctx, st, timing};
-  const Extents mx = {F.W.n_tiles, in->n_tracks, F.W.n_chunks, F.W.n_groups, in->n_unattached, out->probe_state != nullptr};
+  const Extents mx = {F.W.n_tiles, in->n_tracks, F.W.n_chunks, F.W.n_groups, in->n_unattached, out->probe_state != nullptr,
+                      in->n_tracks ? (uint32_t)(in->n_attached / in->n_tracks) : 0u};
   rc = enqueue<false>(ctx, F, nullptr, 1, mx, L);
   ctx->launches = L.n + (validate ? 1 : 0);
   if (rc != TMD_OK) return rc;
@@ -464,13 +481,15 @@ int tmd_decode_batch(tmd_ctx* ctx, uint32_t n_frames, const tmd_compressed* in, 
   const bool timing = (flags & TMD_TIMING) != 0;
   int rc = prepare_timing(ctx, timing);
   if (rc != TMD_OK) return rc;
-  Extents mx = {0, 0, 0, 0, 0, false};
+  Extents mx = {0, 0, 0, 0, 0, false, 0};
   FrameArgs* table = nullptr;
   FrameChunk chunk;
   // Chunk size of the batch: the one a single frame holding ALL the attached clusters would get (larger than any
   // frame's own, so its tables fit the frame's workspace): a batch has chunks enough with every frame cut coarsely.
   uint64_t att_total = 0;
-  for (uint32_t i = 0; i < n_frames; ++i) att_total += in[i].n_attached;
+  uint64_t trk_total = 0;
+  for (uint32_t i = 0; i < n_frames; ++i) { att_total += in[i].n_attached; trk_total += in[i].n_tracks; }
+  mx.mean_len = trk_total ? (uint32_t)(att_total / trk_total) : 0u;
   const uint32_t batch_shift = layout(ctx->geo.n_bins, 0, att_total, ctx->n_sm).chunk_shift;
   auto make_batch_frame = [&](uint32_t i, FrameArgs* F) -> int {
     const int r = make_frame(ctx, &in[i], &out[i], flags, F);
