@@ -86,6 +86,20 @@ def test_adversarial_random_bytes(seed, n_tracks, n_un, max_ncl):
     assert_same(gpu_decode(geo, BZ, c, probe_step=0xFFFFFFFF), O.decode(geo, BZ, c, probe_step=0xFFFFFFFF))
 
 
+@pytest.mark.parametrize("tail", [0, 1, 5, 15, 16, 17, 33, 70])
+def test_every_track_length_at_every_staging_phase(tail):
+    """The decode kernel stages a track's residuals in 16-byte cells of per-stream rings: which cells are
+    staged before the loop, which are requested inside it and which are never needed depends on the track's length and on
+    its first residual index modulo 16.  Lengths 1..100 in a shuffled order put every length at many phases; `tail` is the
+    length of the LAST track, so that the arrays end in the middle of a cell for several remainders (the zero-filled copy
+    that must not read past the arrays) with the last track inside or beyond its pre-staged cells."""
+    geo = build_geometry(36)
+    rng = np.random.default_rng(100 + tail)
+    ncl = np.concatenate([rng.permutation(np.arange(1, 101)) for _ in range(24)] + [np.array([tail + 1])]).astype(np.uint16)
+    c = random_compressed(geo, 0, 300, 200 + tail, ncl=ncl)
+    assert_same(gpu_decode(geo, BZ, c, probe_step=0xFFFFFFFF), O.decode(geo, BZ, c, probe_step=0xFFFFFFFF))
+
+
 def test_empty_and_one_sided_inputs():
     geo = build_geometry(36)
     c = Compressed.empty(0, 0, 0, geo.n_bins)
