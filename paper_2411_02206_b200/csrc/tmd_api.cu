@@ -61,11 +61,19 @@ static_assert(sizeof(FrameChunk) <= 3800, "k_store_frames parameters must fit th
 Workspace layout(uint32_t n_bins, uint32_t n_tracks, uint64_t n_att, int n_sm) {
   Workspace w;
   w.n_tiles = (n_tracks + SCAN_TILE - 1) / SCAN_TILE;
-  // chunk size: the largest power of two that still leaves about one chunk per resident warp of the rank kernel
-  // (20 warps per SM); a pure function of (n_att, SM count), so tmd_workspace_bytes and tmd_decode agree
-  const uint64_t want_chunks = (uint64_t)n_sm * 20;
-  int shift = CHUNK_SHIFT_MIN;
-  while (shift < CHUNK_SHIFT_MAX && (n_att >> (shift + 1)) >= want_chunks) ++shift;
+  // Chunk size (a pure function of (n_att, SM count), so tmd_workspace_bytes and tmd_decode agree).  The rank kernel runs one
+  // warp per chunk, 20 warps per SM: its time goes with ceil(chunks / warps) * chunk size.  The scatter writes one piece per
+  // (chunk, bin): the smaller the chunk the shorter the pieces, measured 14 % per halving (c2, 2^14 -> 2^15: 0.80 -> 0.71 ms).
+  // Cost model in units of "one cluster through the scatter at 2^15": a rank slot costs 6 of them.  Ties go to the larger chunk
+  // (smaller tables).  c3, c4: 2^15; c2: 2^15 (was 2^14 under the round-1 rule "one chunk per resident warp"); c1: 2^11.
+  const uint64_t rank_warps = (uint64_t)n_sm * 20;
+  int shift = CHUNK_SHIFT_MAX;
+  uint64_t best = ~0ull;
+  for (int s = CHUNK_SHIFT_MAX; s >= CHUNK_SHIFT_MIN; --s) {
+    const uint64_t chunks = (n_att + (1ull << s) - 1) >> s, rounds = (chunks + rank_warps - 1) / rank_warps;
+    const uint64_t cost = rounds * (1ull << s) * 600 + n_att * (100 + 14 * (uint64_t)(CHUNK_SHIFT_MAX - s)) / 100;
+    if (cost < best) { best = cost; shift = s; }
+  }
   w.chunk_shift = (uint32_t)shift;
   w.n_chunks = (uint32_t)((n_att + (1ull << shift) - 1) >> shift);
   w.n_groups = (w.n_chunks + COL_GROUP - 1) / COL_GROUP;

@@ -200,6 +200,18 @@ def test_random_bytes_at_the_full_frame_chunk_size():
     _compare_with_oracle(geo, c, "random bytes, shift 15")
 
 
+@pytest.mark.parametrize("n_tracks", [120_000, 220_000, 400_000])
+def test_random_bytes_at_the_intermediate_chunk_sizes(n_tracks):
+    """~12 M, ~22 M and ~40 M attached clusters of random bytes: on a 148-SM device the library's chunk-size rule
+    (csrc/tmd_api.cu, layout) picks chunks of 2^12, 2^13 and 2^14 records for them -- the sizes between the small adversarial inputs
+    (2^11) and the full frames (2^15).  Against the full oracle."""
+    from tmd_inputs import build_geometry
+    from tmd_inputs.adversarial import random_compressed
+    geo = build_geometry(36)
+    c = random_compressed(geo, n_tracks, n_tracks // 2, seed=70 + n_tracks // 100_000, max_ncl=199)
+    _compare_with_oracle(geo, c, f"random bytes, {c.n_attached} attached")
+
+
 def test_whole_chunks_in_one_bin_at_the_full_frame_chunk_size():
     """Tracks of 65 535 clusters that never leave their first bin, half of them sharing one bin: whole 32768-record chunks
     fall into a single bin (u16 histogram / rank / start entries at their limit).  Against the full oracle."""
