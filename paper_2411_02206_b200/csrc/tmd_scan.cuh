@@ -34,6 +34,26 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, ui
   return ws[wid] + inc - v;
 }
 
+// The same for TWO values per thread with one set of barriers (the unattached decode scans pad and time sums together).
+// `ws` = 66 words of shared memory.
+__device__ __forceinline__ void block_excl_scan2(uint32_t a, uint32_t b, uint32_t* ws, uint32_t* ex_a, uint32_t* ex_b, uint32_t* tot_a,
+                                                 uint32_t* tot_b) {
+  const uint32_t lane = lane_id(), wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  const uint32_t ia = warp_incl_scan(a), ib = warp_incl_scan(b);
+  __syncthreads();  // protect ws from a previous call
+  if (lane == 31) { ws[wid] = ia; ws[33 + wid] = ib; }
+  __syncthreads();
+  if (wid == 0) {
+    const uint32_t sa = lane < nw ? ws[lane] : 0, sb = lane < nw ? ws[33 + lane] : 0;
+    const uint32_t sia = warp_incl_scan(sa), sib = warp_incl_scan(sb);
+    ws[lane] = sia - sa; ws[33 + lane] = sib - sb;
+    if (lane == 31) { ws[32] = sia; ws[65] = sib; }
+  }
+  __syncthreads();
+  *tot_a = ws[32]; *tot_b = ws[65];
+  *ex_a = ws[wid] + ia - a; *ex_b = ws[33 + wid] + ib - b;
+}
+
 // ---- A1: off[t] = exclusive prefix sum of trk_ncl (PAPER.md L70 precomputes these indices on the CPU) --------------
 constexpr int SCAN_THREADS = 512;
 constexpr int SCAN_ITEMS = 8;

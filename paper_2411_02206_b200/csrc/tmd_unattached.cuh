@@ -86,8 +86,8 @@ __device__ __forceinline__ void unattached_bin(const DevGeo& G, const Unattached
       tot_p = __shfl_sync(0xffffffffu, inc_p, 31); tot_t = __shfl_sync(0xffffffffu, inc_t, 31);
       ex_p = carry_p + inc_p - sum_p; ex_t = carry_t + inc_t - sum_t;
     } else {
-      ex_p = carry_p + block_excl_scan(sum_p, ws, &tot_p);
-      ex_t = carry_t + block_excl_scan(sum_t, ws, &tot_t);
+      block_excl_scan2(sum_p, sum_t, ws, &ex_p, &ex_t, &tot_p, &tot_t);
+      ex_p += carry_p; ex_t += carry_t;
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -112,7 +112,7 @@ __device__ __forceinline__ void unattached_bin(const DevGeo& G, const Unattached
 template <bool BATCH>
 __global__ void __launch_bounds__(UNATT_THREADS) k_unattached(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
                                                               const FrameArgs* __restrict__ table, uint32_t bins_per_block) {
-  __shared__ uint32_t ws[33];
+  __shared__ uint32_t ws[66];
   const UnattachedArgs A = unattached_args(frame_of<BATCH>(F0, table, blockIdx.y));
   if (A.in.n_unattached == 0) return;
   const uint32_t b0 = blockIdx.x * bins_per_block, b1 = min(b0 + bins_per_block, G.n_bins);
