@@ -44,33 +44,46 @@ __device__ __forceinline__ void unattached_bin(const DevGeo& G, const Unattached
   const uint32_t sec = b / G.n_rows, row = b - sec * G.n_rows;
   const uint32_t tail = (row << 8) | (sec << 16);
   uint32_t carry_p = 0, carry_t = 0;
-  for (uint32_t base = i0 & ~3u; base < i1; base += NT * UNATT_ITEMS) {
-    const uint32_t k0 = base + tid * UNATT_ITEMS;        // multiple of 4
-    uint32_t pd[4] = {0, 0, 0, 0}, td[4] = {0, 0, 0, 0}, qt[4], qm[4], sp[4], st[4], fl[4];
+  // raw words of the four clusters a thread takes from a tile; the NEXT tile's are requested before the current tile is scanned
+  struct Raw { uint2 p2; uint4 t4; uint2 q2, m2; uint32_t a, c, f; };
+  auto load_raw = [&](uint32_t k0) -> Raw {
+    Raw r;
+    r.p2 = make_uint2(0, 0); r.t4 = make_uint4(0, 0, 0, 0); r.q2 = make_uint2(0, 0); r.m2 = make_uint2(0, 0); r.a = r.c = r.f = 0;
     if (k0 < i1 && k0 + 4 > i0) {
       if (k0 + 4 <= n_un) {
-        const uint2 p2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_paddiff + k0));
-        const uint4 t4 = __ldg(reinterpret_cast<const uint4*>(A.in.u_timediff + k0));
-        const uint2 q2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_qtot + k0));
-        const uint2 m2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_qmax + k0));
-        const uint32_t a = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_sigpad + k0));
-        const uint32_t c = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_sigtime + k0));
-        const uint32_t f = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_flags + k0));
-        pd[0] = p2.x & 0xFFFFu; pd[1] = p2.x >> 16; pd[2] = p2.y & 0xFFFFu; pd[3] = p2.y >> 16;
-        td[0] = t4.x; td[1] = t4.y; td[2] = t4.z; td[3] = t4.w;
-        qt[0] = q2.x & 0xFFFFu; qt[1] = q2.x >> 16; qt[2] = q2.y & 0xFFFFu; qt[3] = q2.y >> 16;
-        qm[0] = m2.x & 0xFFFFu; qm[1] = m2.x >> 16; qm[2] = m2.y & 0xFFFFu; qm[3] = m2.y >> 16;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { sp[k] = (a >> (8 * k)) & 0xFFu; st[k] = (c >> (8 * k)) & 0xFFu; fl[k] = (f >> (8 * k)) & 0xFFu; }
+        r.p2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_paddiff + k0));
+        r.t4 = __ldg(reinterpret_cast<const uint4*>(A.in.u_timediff + k0));
+        r.q2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_qtot + k0));
+        r.m2 = __ldg(reinterpret_cast<const uint2*>(A.in.u_qmax + k0));
+        r.a = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_sigpad + k0));
+        r.c = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_sigtime + k0));
+        r.f = __ldg(reinterpret_cast<const uint32_t*>(A.in.u_flags + k0));
       } else {                                                   // the last clusters of the arrays
+        uint32_t pd[4], td[4], qt[4], qm[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const uint32_t i = min(k0 + k, n_un - 1);
           pd[k] = A.in.u_paddiff[i]; td[k] = A.in.u_timediff[i]; qt[k] = A.in.u_qtot[i]; qm[k] = A.in.u_qmax[i];
-          sp[k] = A.in.u_sigpad[i]; st[k] = A.in.u_sigtime[i]; fl[k] = A.in.u_flags[i];
+          r.a |= (uint32_t)A.in.u_sigpad[i] << (8 * k); r.c |= (uint32_t)A.in.u_sigtime[i] << (8 * k); r.f |= (uint32_t)A.in.u_flags[i] << (8 * k);
         }
+        r.p2 = make_uint2(pd[0] | (pd[1] << 16), pd[2] | (pd[3] << 16)); r.t4 = make_uint4(td[0], td[1], td[2], td[3]);
+        r.q2 = make_uint2(qt[0] | (qt[1] << 16), qt[2] | (qt[3] << 16)); r.m2 = make_uint2(qm[0] | (qm[1] << 16), qm[2] | (qm[3] << 16));
       }
     }
+    return r;
+  };
+  Raw nxt = load_raw((i0 & ~3u) + tid * UNATT_ITEMS);
+  for (uint32_t base = i0 & ~3u; base < i1; base += NT * UNATT_ITEMS) {
+    const uint32_t k0 = base + tid * UNATT_ITEMS;        // multiple of 4
+    const Raw cur = nxt;
+    if (base + NT * UNATT_ITEMS < i1) nxt = load_raw(k0 + NT * UNATT_ITEMS);
+    uint32_t pd[4], td[4], qt[4], qm[4], sp[4], st[4], fl[4];
+    pd[0] = cur.p2.x & 0xFFFFu; pd[1] = cur.p2.x >> 16; pd[2] = cur.p2.y & 0xFFFFu; pd[3] = cur.p2.y >> 16;
+    td[0] = cur.t4.x; td[1] = cur.t4.y; td[2] = cur.t4.z; td[3] = cur.t4.w;
+    qt[0] = cur.q2.x & 0xFFFFu; qt[1] = cur.q2.x >> 16; qt[2] = cur.q2.y & 0xFFFFu; qt[3] = cur.q2.y >> 16;
+    qm[0] = cur.m2.x & 0xFFFFu; qm[1] = cur.m2.x >> 16; qm[2] = cur.m2.y & 0xFFFFu; qm[3] = cur.m2.y >> 16;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { sp[k] = (cur.a >> (8 * k)) & 0xFFu; st[k] = (cur.c >> (8 * k)) & 0xFFu; fl[k] = (cur.f >> (8 * k)) & 0xFFu; }
     uint32_t sum_p = 0, sum_t = 0;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
