@@ -94,7 +94,6 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
   // barrier with release semantics (MEMBAR.ALL.GPU + ERRBAR + the wait for the slowest CTA: 26 % of the stall samples).
   __shared__ __align__(8) unsigned long long mbar;
   const uint32_t mbar_addr = (uint32_t)__cvta_generic_to_shared(&mbar);
-  const uint32_t n_valid = __ldg(A.start16 + (size_t)c * A.start_stride + n_bins);      // records of the chunk that have a bin (used late)
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -167,6 +166,7 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
   // ---- wait until this CTA's part of the sorted chunk is complete (phase 0 of the transaction barrier).  The expected byte
   // count is posted only now (the remote completions may come first: the barrier's pending count goes negative meanwhile)
   const uint32_t my_first = rank_in_cluster << per_shift;
+  const uint32_t n_valid = start[n_bins];                           // records of the chunk that have a bin (last entry of the row)
   const uint32_t n_expected = n_valid > my_first ? min(n_valid - my_first, per_cta) : 0u;   // records that land here
   if (tid == 0) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_addr), "r"(n_expected * 16u) : "memory");
   if (n_expected) {
