@@ -98,6 +98,12 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_addr) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // This chunk's row of `rel` is looked up in the write-out phase, a few microseconds from now, in a dependent load in front of
+  // every store: each CTA asks for a sixteenth of it into the L2 now.
+  {
+    const uint32_t row_lines = (n_bins * 4u + 127u) >> 7, per = (row_lines + SC_CLUSTER - 1) / SC_CLUSTER, l = rank_in_cluster * per + tid;
+    if (tid < per && l < row_lines) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const unsigned char*>(A.rel + (size_t)c * n_bins) + l * 128u));
+  }
   // "this CTA is running and its barrier exists": waited for just before the first remote store
   asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");     // (the mbarrier_init fence above is the release it needs)
   // ---- this CTA's share of g: loads in flight before the cluster barrier
