@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
   // ---- this CTA's share of g: loads in flight before the cluster barrier
   const uint32_t g_base = (c << A.chunk_shift) + (rank_in_cluster << per_shift);
   bool first = true;
+  uint32_t local_bytes = 0;                            // bytes of the records this thread stored into its own CTA's part
   for (uint32_t i0 = 0; i0 < per_cta; i0 += SC_THREADS * SC_UNROLL) {
     uint2 rec[SC_UNROLL];
     uint32_t rk[SC_UNROLL], qt[SC_UNROLL], qm[SC_UNROLL], sp[SC_UNROLL], st[SC_UNROLL], fl[SC_UNROLL];
@@ -161,6 +162,11 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
       const uint32_t slot = (uint32_t)start[bin] + rk[k];
       const uint4 v = pack_cluster(rec[k].x, rec[k].y & 0xFFFFu, qt[k], qm[k], sp[k], st[k], fl[k], row, sec);
       const uint32_t dst_cta = slot >> per_shift;
+      if (dst_cta == rank_in_cluster) {                 // stays in this CTA: a plain shared-memory store instead of a request on the
+        recs[slot & (per_cta - 1)] = v;                 // SM's crossbar port (what bounds this kernel); its bytes are counted below
+        local_bytes += 16u;
+        continue;
+      }
       uint32_t r_addr, r_mbar;
       asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r_addr) : "r"(recs_addr + ((slot & (per_cta - 1)) << 4)), "r"(dst_cta));
       asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r_mbar) : "r"(mbar_addr), "r"(dst_cta));
@@ -171,6 +177,7 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
   }
   // ---- wait until this CTA's part of the sorted chunk is complete (phase 0 of the transaction barrier).  The expected byte
   // count is posted only now (the remote completions may come first: the barrier's pending count goes negative meanwhile)
+  if (local_bytes) asm volatile("mbarrier.complete_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(mbar_addr), "r"(local_bytes) : "memory");
   const uint32_t my_first = rank_in_cluster << per_shift;
   const uint32_t n_valid = start[n_bins];                           // records of the chunk that have a bin (last entry of the row)
   const uint32_t n_expected = n_valid > my_first ? min(n_valid - my_first, per_cta) : 0u;   // records that land here
@@ -180,6 +187,7 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
     while (!done)
       asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(mbar_addr) : "memory");
   }
+  __syncthreads();                                     // the locally stored records are visible to every thread of the CTA
   // ---- this CTA's part of the sorted chunk to its canonical positions
   const uint32_t* __restrict__ rel_row = A.rel + (size_t)c * n_bins;
   uint4* __restrict__ out = A.clusters;
