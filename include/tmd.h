@@ -34,7 +34,7 @@ typedef enum {
   TMD_ERR_WORKSPACE = -3, /* workspace missing or smaller than tmd_workspace_bytes()                         */
   TMD_ERR_CUDA = -4,      /* a CUDA runtime call failed (allocation, copy, launch)                           */
   TMD_ERR_CORRUPT = -5,   /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
-  TMD_ERR_DEVICE = -6     /* tmd_create: the device cannot run the kernels (no 16-CTA thread-block clusters)  */
+  TMD_ERR_DEVICE = -6     /* tmd_create: the device cannot run the kernels (no 8-CTA thread-block clusters)  */
 } tmd_status;
 
 #define TMD_MAX_CLUSTERS 0xFFFF0000ull /* n_attached + n_unattached <= this (32-bit indices with headroom for tile overshoot) */

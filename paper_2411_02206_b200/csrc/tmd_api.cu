@@ -825,7 +825,7 @@ const char* tmd_status_string(int status) {
     case TMD_ERR_WORKSPACE: return "workspace missing or too small";
     case TMD_ERR_CUDA: return "CUDA runtime error";
     case TMD_ERR_CORRUPT: return "inconsistent compressed input";
-    case TMD_ERR_DEVICE: return "device cannot run the kernels (thread-block clusters of 16 CTAs)";
+    case TMD_ERR_DEVICE: return "device cannot run the kernels (thread-block clusters of 8 CTAs)";
     default: return "unknown status";
   }
 }

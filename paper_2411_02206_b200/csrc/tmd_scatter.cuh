@@ -49,18 +49,18 @@ __device__ __forceinline__ uint4 pack_cluster(uint32_t T, uint32_t P, uint32_t q
 }
 
 // ---- scatter through distributed shared memory -----------------------------------------------------------------------
-// A thread-block cluster of SC_CLUSTER = 16 CTAs owns one chunk.  The chunk's records are first sorted by (bin, rank) INSIDE
+// A thread-block cluster of SC_CLUSTER = 8 CTAs owns one chunk.  The chunk's records are first sorted by (bin, rank) INSIDE
 // the cluster: record g goes to slot start[bin] + rank16[g] of a 2^chunk_shift-record array that is spread over the shared
-// memories of the 16 CTAs (start = exclusive scan of the chunk's histogram row, from the rank kernel; the store is a DSMEM store,
+// memories of the 8 CTAs (start = exclusive scan of the chunk's histogram row, from the rank kernel; the store is a DSMEM store,
 // st.shared::cluster).  After a cluster barrier every CTA writes its part of the sorted array: records of one bin are now
 // neighbours, so the ~6 records a chunk adds to a bin leave as one contiguous piece and most 32-byte sectors are written
 // whole.  Measured: 16-byte stores that fill half a sector are what bounded the one-thread-per-cluster
 // scatter (a partial-sector write is a read-modify-write in the ECC-protected L2).
-constexpr int SC_CLUSTER = 16;                      // non-portable cluster size (needs cudaFuncAttributeNonPortableClusterSizeAllowed)
-constexpr int SC_CLUSTER_SHIFT = 4;
+constexpr int SC_CLUSTER = 8;                       // CTAs per cluster.  Measured at c3: 16 CTAs x 2048 records, 5 CTAs per SM 2.64 ms (a cluster of 16 needs
+constexpr int SC_CLUSTER_SHIFT = 3;                 // 16 free CTA slots in ONE GPC: 38 resident clusters = 608 of 740 slots); 8 x 4096, 3 per SM 2.54; 4 x 8192 4.10
 constexpr int SC_THREADS = 256;
 constexpr int SC_UNROLL = 4;                       // records per thread and batch (the vector loads below are written for 4)
-constexpr uint32_t SC_MAX_PER_CTA = (1u << CHUNK_SHIFT_MAX) / SC_CLUSTER;   // 2048 records = 32 KB
+constexpr uint32_t SC_MAX_PER_CTA = (1u << CHUNK_SHIFT_MAX) / SC_CLUSTER;   // 4096 records = 64 KB
 
 __host__ __device__ inline size_t sc_smem_bytes(uint32_t n_bins) { return (size_t)SC_MAX_PER_CTA * 16 + (size_t)sc_start_stride(n_bins) * 2; }
 
@@ -76,7 +76,7 @@ __device__ __forceinline__ ScatterArgs scatter_args(const FrameArgs& F, uint32_t
 }
 
 template <bool BATCH>
-__global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
+__global__ void __launch_bounds__(SC_THREADS, 3) k_scatter(const __grid_constant__ DevGeo G, const __grid_constant__ FrameArgs F0,
                                                            const FrameArgs* __restrict__ table) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const FrameArgs& F = frame_of<BATCH>(F0, table, blockIdx.y);
@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(SC_THREADS, 5) k_scatter(const __grid_constant
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   // This chunk's row of `rel` is looked up in the write-out phase, a few microseconds from now, in a dependent load in front of
-  // every store: each CTA asks for a sixteenth of it into the L2 now.
+  // every store: each CTA asks for its share of it into the L2 now.
   {
     const uint32_t row_lines = (n_bins * 4u + 127u) >> 7, per = (row_lines + SC_CLUSTER - 1) / SC_CLUSTER, l = rank_in_cluster * per + tid;
     if (tid < per && l < row_lines) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const unsigned char*>(A.rel + (size_t)c * n_bins) + l * 128u));
