@@ -34,7 +34,8 @@ typedef enum {
   TMD_ERR_WORKSPACE = -3, /* workspace missing or smaller than tmd_workspace_bytes()                         */
   TMD_ERR_CUDA = -4,      /* a CUDA runtime call failed (allocation, copy, launch)                           */
   TMD_ERR_CORRUPT = -5,   /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
-  TMD_ERR_DEVICE = -6     /* tmd_create: the device cannot run the kernels (no 8-CTA thread-block clusters)  */
+  TMD_ERR_DEVICE = -6,    /* tmd_create: the device cannot run the kernels (no 8-CTA thread-block clusters)  */
+  TMD_ERR_LIMIT = -7      /* tmd_decode_unattached_noalloc: the sizes exceed its fixed, built-in scratch      */
 } tmd_status;
 
 #define TMD_MAX_CLUSTERS 0xFFFF0000ull /* n_attached + n_unattached <= this (32-bit indices with headroom for tile overshoot) */
@@ -196,6 +197,41 @@ int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uin
 #define TMD_HOST_SLOTS 2
 int tmd_decode_host_async(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot);
 int tmd_host_wait(tmd_ctx* ctx, int slot);
+
+/*
+ * Unattached clusters only (row A7 with the bin offsets of A4, second kernel: "computes each coordinate
+ * summing the difference taken from the input array with the coordinates of the last decoded cluster"), for callers that
+ * MAY NOT ALLOCATE device memory -- neither here nor at set-up.  Typical cases: the library runs inside a framework that
+ * claimed the whole device memory as one block at start-up and rules out any later cudaMalloc; the caller is a plug-in that
+ * only ever sees device pointers handed to it; the call sits in a loop that cannot afford the device-wide serialisation of
+ * cudaMalloc / cudaFree.  Such a caller cannot use tmd_create (it allocates the geometry table) or provide a workspace, so
+ * this call takes neither: no context, no workspace, and it calls no cudaMalloc, cudaFree or other allocating routine.
+ *
+ * Its scratch (the per-bin start table, 4 bytes x 2 per bin) is a fixed array of 65 792 bytes compiled into libtmd.so;
+ * every GPU on which the library's code is loaded holds that array from then until the process exits, used or not.
+ * Hence the limit: n_sectors_out * n_rows <= TMD_NOALLOC_MAX_BINS, else TMD_ERR_LIMIT (also for n_unattached >
+ * TMD_MAX_CLUSTERS); nothing is enqueued for a refused call.
+ *
+ *   n_sectors_out, n_rows : the bin grid, bin = sector * n_rows + row (n_rows <= 255), as in tmd_geometry;
+ *   in        : HOST struct; n_tracks and n_attached must be 0 (TMD_ERR_ARG otherwise: attached clusters need tmd_decode);
+ *               u_bin_count [n_bins] and the seven u_* arrays [n_unattached] are DEVICE pointers, 16-byte aligned,
+ *               caller-owned, read-only; the trk_* / a_* members are ignored;
+ *   clusters  : DEVICE [n_unattached], 16-byte aligned, written; bin after bin, each bin in stored order;
+ *   bin_offset: DEVICE [n_bins + 1], written;
+ *   both outputs equal, byte for byte, what tmd_decode writes for the same frame.
+ * Enqueues two kernels on `cuda_stream` and returns; results are valid once the stream has been synchronised.
+ *
+ * Set-up: the FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, with the caller's
+ * current device; checked, TMD_ERR_CUDA on failure) and remembers it per device.  Make that first call during
+ * initialisation, before any stream capture begins on that device.
+ * Sharing: all calls on one device use the same array, and it keeps what the previous call left there.  Each call rewrites
+ * every entry it will read (including the part that must be zero) before reading it, so calls that run one after the other
+ * -- same stream, or ordered by events -- are independent of each other.  Two calls whose kernels can overlap on the GPU
+ * (different streams or host threads, no ordering between them) RACE on the array: the results of both are undefined.
+ */
+#define TMD_NOALLOC_MAX_BINS 8192u
+int tmd_decode_unattached_noalloc(uint32_t n_sectors_out, uint32_t n_rows, const tmd_compressed* in, tmd_cluster* clusters,
+                                  uint32_t* bin_offset, void* cuda_stream);
 
 /*
  * Self test of the arithmetic the track-decode kernel relies on (every model operation is ONE IEEE-754

@@ -826,6 +826,7 @@ const char* tmd_status_string(int status) {
     case TMD_ERR_CUDA: return "CUDA runtime error";
     case TMD_ERR_CORRUPT: return "inconsistent compressed input";
     case TMD_ERR_DEVICE: return "device cannot run the kernels (thread-block clusters of 8 CTAs)";
+    case TMD_ERR_LIMIT: return "sizes exceed the built-in scratch of the no-allocation entry point";
     default: return "unknown status";
   }
 }

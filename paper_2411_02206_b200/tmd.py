@@ -15,7 +15,8 @@ from . import build as _build
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
-TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT, TMD_ERR_DEVICE = 0, -1, -2, -3, -4, -5, -6
+TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_CORRUPT, TMD_ERR_DEVICE, TMD_ERR_LIMIT = 0, -1, -2, -3, -4, -5, -6, -7
+TMD_NOALLOC_MAX_BINS = 8192
 TMD_VALIDATE = 1
 TMD_TIMING = 2
 TMD_SERIAL = 4
@@ -93,6 +94,8 @@ def lib() -> C.CDLL:
         L.tmd_entropy_decode.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p, C.c_size_t, C.POINTER(tmd_compressed), C.c_void_p, C.c_void_p]
         for f in (L.tmd_entropy_bound, L.tmd_entropy_encode_host, L.tmd_entropy_sizes, L.tmd_entropy_decode):
             f.restype = C.c_int
+        L.tmd_decode_unattached_noalloc.argtypes = [C.c_uint32, C.c_uint32, C.POINTER(tmd_compressed), C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tmd_decode_unattached_noalloc.restype = C.c_int
         L.tmd_selftest_ieee.argtypes = [C.c_uint32, C.POINTER(C.c_uint64)]
         L.tmd_selftest_ieee.restype = C.c_int
         L.tmd_decode_host_async.restype = C.c_int
@@ -205,6 +208,14 @@ def tmd_decode_host_async(ctx: int, comp: tmd_compressed, out: tmd_output, flags
 def tmd_host_wait(ctx: int, slot: int = 0) -> None:
     """Block until the frame in pipeline slot `slot` is complete in its host buffers."""
     _check(lib().tmd_host_wait(ctx, slot))
+
+
+def tmd_decode_unattached_noalloc(n_sectors_out: int, n_rows: int, comp: tmd_compressed, clusters, bin_offset, stream: int = 0) -> None:
+    """Enqueue the decode of a frame that holds only unattached clusters, for callers that cannot allocate device memory
+    (no context, no workspace: the scratch is a fixed array inside libtmd.so; at most TMD_NOALLOC_MAX_BINS bins, else
+    TmdError(TMD_ERR_LIMIT)).  `comp.u_*`, `clusters`, `bin_offset`: DEVICE memory.  Calls on one device share the scratch:
+    keep them ordered (one stream, or events); see include/tmd.h."""
+    _check(lib().tmd_decode_unattached_noalloc(n_sectors_out, n_rows, C.byref(comp), _ptr(clusters), _ptr(bin_offset), stream))
 
 
 def tmd_selftest_ieee(log2_pairs: int = 32) -> tuple[int, int, int]:
