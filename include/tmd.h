@@ -35,7 +35,8 @@ typedef enum {
   TMD_ERR_CUDA = -4,      /* a CUDA runtime call failed (allocation, copy, launch)                           */
   TMD_ERR_CORRUPT = -5,   /* TMD_VALIDATE only: counts / first-cluster fields are inconsistent               */
   TMD_ERR_DEVICE = -6,    /* tmd_create: the device cannot run the kernels (no 8-CTA thread-block clusters)  */
-  TMD_ERR_LIMIT = -7      /* tmd_decode_unattached_noalloc: the sizes exceed its fixed, built-in scratch      */
+  TMD_ERR_LIMIT = -7      /* a fixed built-in size is exceeded: the scratch of tmd_decode_unattached_noalloc,
+                             the 4 GiB of a TMDZ container (tmd_entropy_encode_host)                          */
 } tmd_status;
 
 #define TMD_MAX_CLUSTERS 0xFFFF0000ull /* n_attached + n_unattached <= this (32-bit indices with headroom for tile overshoot) */
@@ -254,9 +255,10 @@ const char* tmd_status_string(int status);
 int tmd_last_launch_count(const tmd_ctx* ctx);
 
 /*
- * Per-kernel device times of the last tmd_decode that ran with TMD_TIMING: waits for that call's last event, then
- * fills names[i] (static strings) and ms[i] for its kernels in launch order.  Returns the number filled (0 if the last
- * call did not use TMD_TIMING) or a negative tmd_status.
+ * Per-kernel device times of the last tmd_decode / tmd_decode_batch that ran with TMD_TIMING: waits for that call's last
+ * event, then fills names[i] (static strings) and ms[i] for its kernels in launch order.  Returns the number filled (0 if
+ * the last call did not use TMD_TIMING) or a negative tmd_status.  A batch reports the upload of its frame table (one
+ * small launch per 8 frames) as a single row "store_frames", so the rows never exceed TMD_MAX_KERNELS.
  */
 int tmd_kernel_times(tmd_ctx* ctx, int max_kernels, const char** names, float* ms);
 
@@ -305,7 +307,10 @@ int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster
  * tmd_entropy_bound:       upper bound of the container size for these counts.
  * tmd_entropy_encode_host: HOST arrays in (`in`: host pointers), TMDZ container out (`blob`, HOST, capacity >= the bound).
  *                          Runs on the calling host thread (the paper's rANS encoding is a CPU step of the synchronous
- *                          phase, L40).
+ *                          phase, L40).  A container is limited to 4 GiB (block positions are 32-bit byte offsets from
+ *                          its start): TMD_ERR_LIMIT when the coded data passes that, `blob` is then unspecified.  The
+ *                          bound is not the test (it assumes incompressible data): a full Pb-Pb frame, 4.8 GB of
+ *                          arrays, codes to about 2.1 GB.
  * tmd_entropy_sizes:       counts stored in a container's header (`head` = at least its first 64 bytes, HOST).
  * tmd_entropy_decode:      decodes a container resident in DEVICE memory (`d_blob`, 16-byte aligned) into the DEVICE arrays
  *                          `out` points to (caller-allocated with the counts of tmd_entropy_sizes, 16-byte aligned; out's
@@ -313,8 +318,12 @@ int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster
  *                          container's first 64 + 32 * 43 bytes (header + plane directory; the caller read the container
  *                          from storage through host memory anyway).  Only enqueues one kernel on `cuda_stream`; one CTA
  *                          decodes eight blocks (one per warp) and assembles 64 KiB of one array.  `d_err4` = 4 bytes of
- *                          DEVICE memory that are non-zero afterwards if a table does not sum to 4096 or a block is too
- *                          short (corrupt container; the output is then unspecified but nothing is written out of bounds).
+ *                          DEVICE memory that are non-zero afterwards if the container is corrupt (bit 0: a table does
+ *                          not sum to 4096; bit 1: a block is shorter than its symbols need; bit 2: a block position is
+ *                          out of order, out of bounds or misaligned; bit 3: a block's coder states do not return to
+ *                          their start value or words are left over, i.e. its data was altered); the output is then
+ *                          unspecified but nothing is read or written out of bounds.  A plane directory that points
+ *                          outside the container is refused on the host (TMD_ERR_CORRUPT).
  *                          The arrays can be handed to tmd_decode on the same stream right away.
  */
 int tmd_entropy_bound(uint32_t n_tracks, uint64_t n_attached, uint64_t n_unattached, uint32_t n_bins, size_t* out_bytes);

@@ -523,13 +523,20 @@ int tmd_decode_batch(tmd_ctx* ctx, uint32_t n_frames, const tmd_compressed* in, 
     mx.any_probe = mx.any_probe || out[i].probe_state != nullptr;
   }
   Launcher L{ctx, st, timing};
+  // The frame table goes up STORE_FRAMES entries per launch.  With TMD_TIMING the whole upload is ONE timed row
+  // ("store_frames"): a pair per launch would use up the TMD_MAX_KERNELS pairs at ~100 frames and push the decode
+  // kernels off the end of tmd_kernel_times.
+  int store_launches = 0;
+  if (!L.before()) return TMD_ERR_CUDA;
   for (uint32_t first = 0; first < n_frames; first += STORE_FRAMES) {
     const uint32_t count = n_frames - first < STORE_FRAMES ? n_frames - first : STORE_FRAMES;
     for (uint32_t k = 0; k < count; ++k) make_batch_frame(first + k, &chunk.f[k]);
-    TMD_LAUNCH("store_frames", k_store_frames<<<1, 256, 0, st>>>(chunk, table, first, count));
+    k_store_frames<<<1, 256, 0, st>>>(chunk, table, first, count);
+    ++store_launches;
   }
+  if (!L.after("store_frames")) return TMD_ERR_CUDA;
   rc = enqueue<true>(ctx, chunk.f[0], table, n_frames, mx, L);
-  ctx->launches = L.n;
+  ctx->launches = L.n + store_launches - 1;      // L counted the upload as one
   if (rc != TMD_OK) return rc;
   ctx->timed_launches = L.n;
   ctx->timing_valid = timing;
@@ -651,12 +658,7 @@ int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster
   TMD_CUDA(cudaStreamSynchronize(st));
   if (h_err[ERR_TRACK_FIELD]) return TMD_ERR_CORRUPT;       // a row / sector without an output bin
   if (n_un == 0) return TMD_OK;
-  static bool smem_set = false;
-  if (!smem_set) {
-    TMD_CUDA(allow_smem(k_un_sort_tiles, (size_t)UN_TILE * 16));
-    TMD_CUDA(allow_smem(k_un_merge, (size_t)UN_TILE * 16));
-    smem_set = true;
-  }
+  static_assert((size_t)UN_TILE * 16 <= 48 * 1024, "below the default dynamic shared-memory limit: no per-function attribute needed");
   const uint32_t tile_bound = n_un / UN_TILE + n_bins;      // >= number of tiles; surplus blocks return at once
   k_un_bucket<<<stream_blocks, 256, 0, st>>>(A);
   k_un_sort_tiles<<<tile_bound, UN_THREADS, (size_t)UN_TILE * 16, st>>>(A);

@@ -107,7 +107,8 @@ __global__ void __launch_bounds__(Z_THREADS) k_entropy_decode(const __grid_const
   if (n) {
     const uint32_t* starts = reinterpret_cast<const uint32_t*>(Z.blob + Z.pl[A.first_plane + j].blocks_offset);
     uint32_t s0 = starts[b], s1 = starts[b + 1];
-    if (s1 < s0 || s1 > Z.blob_bytes || s1 - s0 < 4 * Z_LANES) {               // corrupt block table: decode nothing from it
+    if (s1 < s0 || s1 > Z.blob_bytes || s1 - s0 < 4 * Z_LANES || (s0 & 3u)) {   // corrupt block table (out of order, out of bounds,
+                                                                               // too short, states not 4-byte aligned): decode nothing from it
       if (lane == 0) atomicOr(&err[0], 4u);
       s0 = 0; s1 = 4 * Z_LANES;
     }
@@ -184,7 +185,15 @@ __global__ void __launch_bounds__(Z_THREADS) k_entropy_decode(const __grid_const
     }
     __syncthreads();
   }
-  if (n && lane == 0 && used > max_words) atomicOr(&err[0], 2u);               // a block shorter than its symbols need
+  if (n) {
+    // The encoder starts every coder at Z_L and the decoder undoes its steps exactly, so an intact block leaves all 32 states at
+    // Z_L (coders without a symbol never moved) and has consumed every word but at most the one that pads the block to 4 bytes.
+    const bool off_end = __any_sync(0xffffffffu, x != Z_L);
+    if (lane == 0) {
+      if (used > max_words) atomicOr(&err[0], 2u);                              // a block shorter than its symbols need
+      else if (off_end || max_words - used > 1u) atomicOr(&err[0], 8u);         // damaged words or states (bit flips inside the block)
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------- host side
@@ -304,7 +313,7 @@ int tmd_entropy_encode_host(const tmd_compressed* in, uint32_t n_bins, void* blo
       pos += 4 * (blocks + 1);
       for (uint64_t b = 0; b < blocks; ++b) {
         align_to(4);
-        if (pos > 0xFFFFFFFFull) return TMD_ERR_ARG;                     // block starts are 32-bit: containers stay below 4 GiB
+        if (pos > 0xFFFFFFFFull) return TMD_ERR_LIMIT;                   // block starts are 32-bit: containers stay below 4 GiB
         wr32(out + starts_off + 4 * b, (uint32_t)pos);
         const uint64_t first = b * Z_BLOCK;
         const uint32_t m = (uint32_t)std::min<uint64_t>(Z_BLOCK, n - first);
@@ -320,7 +329,7 @@ int tmd_entropy_encode_host(const tmd_compressed* in, uint32_t n_bins, void* blo
         for (size_t i = rev.size(); i-- > 0;) { memcpy(out + pos, &rev[i], 2); pos += 2; }
       }
       align_to(4);
-      if (pos > 0xFFFFFFFFull) return TMD_ERR_ARG;
+      if (pos > 0xFFFFFFFFull) return TMD_ERR_LIMIT;
       wr32(out + starts_off + 4 * blocks, (uint32_t)pos);
       unsigned char* d = out + Z_HEADER + (uint64_t)Z_PLANE * p_index;
       wr32(d, a); wr32(d + 4, j); wr64(d + 8, n); wr64(d + 16, table_off); wr64(d + 24, starts_off);
@@ -381,20 +390,17 @@ int tmd_entropy_decode(const void* head, size_t head_bytes, const void* d_blob, 
       if (rd32(d) != a || rd32(d + 4) != j || rd64(d + 8) != n) return TMD_ERR_CORRUPT;
       Z.pl[p_index].table_offset = rd64(d + 16);
       Z.pl[p_index].blocks_offset = rd64(d + 24);
-      if (Z.pl[p_index].table_offset + 512 > h.total || Z.pl[p_index].blocks_offset + 4 * (blocks + 1) > h.total ||
-          (Z.pl[p_index].table_offset & 1u) || (Z.pl[p_index].blocks_offset & 3u))
+      // (written without sums that could wrap for offsets near 2^64)
+      const uint64_t t_off = Z.pl[p_index].table_offset, b_off = Z.pl[p_index].blocks_offset, starts_bytes = 4 * (blocks + 1);
+      if (t_off > h.total || h.total - t_off < 512 || b_off > h.total || h.total - b_off < starts_bytes || (t_off & 1u) || (b_off & 3u))
         return TMD_ERR_CORRUPT;
     }
   }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (cudaMemsetAsync(d_err4, 0, 4, st) != cudaSuccess) return TMD_ERR_CUDA;
   if (chunk == 0) return TMD_OK;
-  const size_t smem = (size_t)Z_WARPS * Z_PART + 4 * (size_t)Z_M + 4 * 256 * 4;
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(k_entropy_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return TMD_ERR_CUDA;
-    attr_set = true;
-  }
+  constexpr size_t smem = (size_t)Z_WARPS * Z_PART + 4 * (size_t)Z_M + 4 * 256 * 4;
+  static_assert(smem <= 48 * 1024, "below the default dynamic shared-memory limit: no per-function attribute (and no per-process flag) needed");
   k_entropy_decode<<<chunk, Z_THREADS, smem, st>>>(Z, (uint32_t*)d_err4);
   return cudaGetLastError() == cudaSuccess ? TMD_OK : TMD_ERR_CUDA;
 }

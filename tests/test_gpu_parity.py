@@ -304,6 +304,21 @@ def test_batch_of_frames_equals_frame_by_frame():
             assert_same(got, (w_cl, w_bo, w_pr if d_pr is not None else None))
         with pytest.raises(T.TmdError):                      # TMD_VALIDATE synchronises: not accepted for a batch
             T.tmd_decode_batch(ctx, T.make_batch(comps, outs), T.TMD_VALIDATE, 0)
+        # TMD_TIMING on a batch whose frame table needs many upload launches (19 frames x 11 = 209 frames -> 27 launches, more
+        # than the TMD_MAX_KERNELS event pairs): the upload is one row and every decode kernel is still reported
+        more = []
+        for rep in range(10):                                # the same inputs again, every frame with outputs and workspace of its own
+            for c, (dev, d_cl, d_bo, d_pr, ws) in zip(frames, held):
+                bufs = (torch.empty_like(d_cl), torch.empty_like(d_bo), torch.empty_like(ws))
+                held.append(bufs)                            # tmd_output holds addresses only: keep the tensors alive
+                more.append(T.make_output(*bufs))
+        many = T.make_batch(comps * 11, outs + more)
+        T.tmd_decode_batch(ctx, many, T.TMD_TIMING, torch.cuda.current_stream().cuda_stream)
+        rows = T.tmd_kernel_times(ctx)
+        names = [r[0] for r in rows]
+        assert names.count("store_frames") == 1 and names[0] == "store_frames" and names[-1] == "scatter" and len(rows) == 13
+        assert T.tmd_last_launch_count(ctx) == 12 + 27
+        torch.cuda.synchronize()
     finally:
         T.tmd_destroy(ctx)
 
@@ -492,3 +507,26 @@ def test_entropy_decode_edge_cases_and_library_encoder():
     assert _gpu_entropy_decode(bad)[1] & 1
     bad = blob.copy(); bad[b_off:b_off + 8].view(np.uint32)[:] = (0xFFFFFF00, 5)
     assert _gpu_entropy_decode(bad)[1] & 4
+    # a block position that is in order and in bounds but not 4-byte aligned (its 32 states are read as words): reported,
+    # not followed into a misaligned-address fault that would poison the CUDA context for every later test
+    starts = blob[b_off:b_off + 8].view(np.uint32)
+    for shift in (1, 2, 3):
+        bad = blob.copy(); bad[b_off:b_off + 4].view(np.uint32)[0] = starts[0] + shift
+        assert _gpu_entropy_decode(bad)[1] & 4, shift
+    # bit flips inside a block: one of its words, one of its coder states
+    s0, s1 = int(starts[0]), int(starts[1])
+    assert s1 - s0 > 4 * 32 + 64
+    bad = blob.copy(); bad[s0 + 4 * 32 + 40] ^= 0x10
+    assert _gpu_entropy_decode(bad)[1] & (8 | 2)
+    bad = blob.copy(); bad[s0 + 4 * 7 + 1] ^= 0x01
+    assert _gpu_entropy_decode(bad)[1] & (8 | 2)
+    # a plane directory that points far outside the container (offsets near 2^64 must not wrap the host's range check)
+    for field in (16, 24):
+        for v in (0xFFFFFFFFFFFFFF00, 0xFFFFFFFFFFFFFFFC, blob.size, blob.size - 4):
+            bad = blob.copy(); bad[64 + field:64 + field + 8].view(np.uint64)[0] = v
+            with pytest.raises(T.TmdError) as e:
+                _gpu_entropy_decode(bad)
+            assert e.value.status == T.TMD_ERR_CORRUPT, (field, hex(v))
+    out, err = _gpu_entropy_decode(blob)                    # the context survived all of the above
+    assert err == 0
+    _assert_arrays_equal(out, c)
