@@ -23,8 +23,10 @@
  * sums and the canonical order; decode(encode(x)) == x; brute-force checks on tiny inputs; and, for every branch of
  * orc_init / orc_step (the `!ok` path, multi-step rotations, the saturation constants, reading 19's reductions), an
  * independent numpy-float32 evaluation of the op list (tests/c3_numpy.py, tests/test_oracle_independent.py) compared
- * per step on all 20 trace columns.  DESIGN.md §4 lists mutation -> failing test.  No function here is "parity
- * unpinned".
+ * per step on all 20 trace columns; the encoder's own lines (trk_qpt rounding / clamp, the unattached sort key) by
+ * hand-worked values and numpy.lexsort, the short-step branch with dx != 0 by constructed tracks, the whole file under
+ * ASan + UBSan (tests/test_oracle_encoder_pins.py).  DESIGN.md §4 lists mutation -> failing test.  No function here is
+ * "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
