@@ -365,6 +365,40 @@ def side_workload(T, name: str, device, steps: int, peak: float) -> dict:
             "l2": "inputs larger than L2, no flush" if fr.algorithmic_bytes() > 400e6 else "L2-resident workload (flag)"}
 
 
+def two_in_flight(T, ctx, geo, arrays, device, steps: int, one_frame_ms: float) -> dict:
+    """"multiple instances are executed concurrently on different streams".  Two time frames (the same
+    compressed arrays, read-only; outputs and workspace of their own) decoded by two plain tmd_decode calls per step on two
+    streams, so that one frame's memory-bound kernels can run beside the other's issue-bound track decode.  Measured twice:
+    both streams at the default priority, and the second stream at high priority.  value = clusters of both frames over the
+    time from the common start to the later of the two ends (CUDA events)."""
+    import torch
+    frames = [Frame(T, ctx, geo, arrays, device) for _ in range(2)]
+    out = {"frames_in_flight": 2, "steps": steps, "one_frame_at_a_time_ms": one_frame_ms}
+    cur = torch.cuda.current_stream()
+    for label, prio in (("equal_priority", 0), ("second_stream_high_priority", -1)):
+        streams = [torch.cuda.Stream(device=device, priority=0), torch.cuda.Stream(device=device, priority=prio)]
+
+        def run(k: int) -> float:
+            torch.cuda.synchronize()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record(cur)
+            for st, fr in zip(streams, frames):
+                st.wait_event(t0)
+                for _ in range(k):
+                    T.tmd_decode(ctx, fr.comp, fr.out, 0, st.cuda_stream)
+                cur.wait_stream(st)
+            t1.record(cur)
+            torch.cuda.synchronize()
+            return t0.elapsed_time(t1)
+        run(3)
+        ms = run(steps) / steps                               # per pair of frames
+        out[label] = {"ms_per_two_frames": ms, "value": 2 * frames[0].n_cl / (ms * 1e-3), "unit": UNIT,
+                      "speedup_vs_one_at_a_time": 2 * one_frame_ms / ms}
+    del frames
+    torch.cuda.empty_cache()
+    return out
+
+
 def batch_workload(T, device, n_frames: int, steps: int, peak: float) -> dict | None:
     """n_frames c1-sized frames (single Pb-Pb-like events, different seeds) decoded by ONE
     tmd_decode_batch call, next to the same frames decoded one tmd_decode call after the other."""
@@ -404,14 +438,15 @@ def batch_workload(T, device, n_frames: int, steps: int, peak: float) -> dict | 
             "l2": "each frame is L2-sized; 64 frames = 3 GB of traffic per step, no flush"}
 
 
-def entropy_workload(T, device, steps: int, peak: float) -> dict | None:
-    """the entropy stage in front (PAPER.md L49 'TPC Entropy Decoding').  One eighth of a c2 frame is
-    written as a TMDZ container by the library's HOST encoder (one core, outside any timed region), copied to the device,
-    and the GPU rANS decode into the compressed SoA is timed alone and chained with tmd_decode on the same stream."""
+def entropy_workload(T, device, steps: int, peak: float, workload: str) -> dict | None:
+    """the entropy stage in front (PAPER.md L49 'TPC Entropy Decoding').  The WHOLE frame of `workload`
+    (c3: 4.8 GB of arrays, a ~2.1 GB container) is written as a TMDZ container by the library's HOST encoder (one core,
+    outside any timed region, ~20 s at c3), copied to the device, and the GPU rANS decode into the compressed SoA is timed
+    alone and chained with tmd_decode on the same stream."""
     import torch
     if not hasattr(T, "tmd_entropy_decode"):
         return None
-    geo, arrays = build_workload("c2", device, scale=0.125)
+    geo, arrays = build_workload(workload, device)
     host = {k: v.cpu() for k, v in arrays.items()}
     t0 = time.perf_counter()
     blob = T.tmd_entropy_encode_host(host, geo.n_bins)
@@ -431,27 +466,83 @@ def entropy_workload(T, device, steps: int, peak: float) -> dict | None:
         T.tmd_entropy_decode(head, d_blob, out, d_err, stream)
         T.tmd_decode(ctx, fr.comp, fr.out, 0, stream)
     ms_c = timed_steps(chain, steps, 3, torch.cuda.synchronize)
-    T.tmd_destroy(ctx)
     sz, sc = stats(ms_z), stats(ms_c)
-    return {"workload": "one eighth of c2", "n_attached": fr.n_att, "n_unattached": fr.n_un, "raw_bytes": raw, "container_bytes": int(blob.size),
+    n_att_, n_un_, n_cl_ = fr.n_att, fr.n_un, fr.n_cl
+    # ---- container in, clusters out, host to host (tmd_decode_container_host_async): the e2e leg again, with the 2.3x smaller
+    #      container on the bus instead of the arrays; same two-slot pipeline, same wall-clock timing, copies inside
+    del fr, out, arrays, d_blob
+    torch.cuda.empty_cache()
+    h_blob = torch.from_numpy(blob).pin_memory()
+    keep, houts = [], []
+    for _ in range(T.TMD_HOST_SLOTS):
+        hc = torch.empty(n_cl_ * 16, dtype=torch.uint8, pin_memory=True)
+        hb = torch.empty(geo.n_bins + 1, dtype=torch.int32, pin_memory=True)
+        keep.append((hc, hb)); houts.append(T.make_output(hc, hb))
+    for s_ in range(T.TMD_HOST_SLOTS):
+        T.tmd_decode_container_host_async(ctx, h_blob, houts[s_], 0, s_)
+    for s_ in range(T.TMD_HOST_SLOTS):
+        T.tmd_host_wait(ctx, s_)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(steps):
+        T.tmd_decode_container_host_async(ctx, h_blob, houts[i % T.TMD_HOST_SLOTS], 0, i % T.TMD_HOST_SLOTS)
+    for s_ in range(T.TMD_HOST_SLOTS):
+        T.tmd_host_wait(ctx, s_)
+    pipe_s = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    T.tmd_decode_container_host_async(ctx, h_blob, houts[0], 0, 0)
+    T.tmd_host_wait(ctx, 0)
+    single_s = time.perf_counter() - t0
+    e2e_container = {"value": n_cl_ * steps / pipe_s, "unit": UNIT, "h2d_bytes_per_step": int(h_blob.numel()),
+                     "d2h_bytes_per_step": int(keep[0][0].numel() + keep[0][1].numel() * 4), "steps": steps,
+                     "mode": "two-slot pipeline, tmd_decode_container_host_async (upload container, entropy decode, decode, download)",
+                     "single_frame_ms": 1e3 * single_s}
+    T.tmd_destroy(ctx)
+    del keep, houts, h_blob
+    return {"workload": f"full {workload} frame", "e2e_container": e2e_container, "n_attached": n_att_, "n_unattached": n_un_, "raw_bytes": raw, "container_bytes": int(blob.size),
             "compression": raw / blob.size, "restores_the_arrays": bool(same), "entropy_decode_ms": sz["mean"], "entropy_decode_ms_min": sz["min"],
             "entropy_decode_out_gbs": raw / (sz["mean"] * 1e-3) / 1e9, "entropy_decode_frac_of_hbm_peak": (raw + blob.size) / (sz["mean"] * 1e-3) / 1e9 / peak,
-            "chain_ms": sc["mean"], "chain_clusters_per_s": fr.n_cl / (sc["mean"] * 1e-3), "host_encode_s": enc_s,
-            "l2": "container (%.0f MB) + arrays (%.0f MB): partly L2-resident (flag)" % (blob.size / 1e6, raw / 1e6)}
+            "chain_ms": sc["mean"], "chain_clusters_per_s": n_cl_ / (sc["mean"] * 1e-3), "host_encode_s": enc_s,
+            "l2": "container (%.0f MB) + arrays (%.0f MB): %s" % (blob.size / 1e6, raw / 1e6, "larger than L2, no flush"
+                                                                  if blob.size + raw > 400e6 else "partly L2-resident (flag)")}
+
+
+KERNEL_SOURCES = ("tmd_api.cu", "tmd_common.cuh", "tmd_decode.cuh", "tmd_rank.cuh", "tmd_scan.cuh", "tmd_scatter.cuh", "tmd_sort.cuh",
+                  "tmd_unattached.cuh")
+
+
+def kernel_source_hash() -> str:
+    """sha256 (first 12 hex digits) over the sources of the kernels of one tmd_decode step and their launch code: the key that
+    ties profiles/traffic.txt (numbers read from an ncu capture) to the tree they were captured from."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        h.update(open(os.path.join(ROOT, "paper_2411_02206_b200", "csrc", name), "rb").read())
+    return h.hexdigest()[:12]
 
 
 def ncu_profile_numbers(kernel: str, workload: str):
-    """(dram bytes per launch, warp instructions per launch, source file) of `kernel` from the committed ncu summary
-    (profiles/traffic.txt: workload kernel dram_bytes warp_inst), else (None, None, None)."""
+    """(dram bytes per launch, warp instructions per launch, observed bound, source) of `kernel` from the committed ncu summary
+    profiles/traffic.txt (`workload kernel dram_bytes warp_inst observed-bound...`; a line `sources <hash>` names the kernel
+    sources the capture was made from).  If the kernels changed since (hash differs), the numbers are REFUSED: (None, None,
+    None, reason)."""
     path = os.path.join(ROOT, "profiles", "traffic.txt")
+    found, captured = None, None
     try:
         for line in open(path):
             v = line.split()
+            if len(v) >= 2 and v[0] == "sources":
+                captured = v[1]
             if len(v) >= 3 and v[0] == workload and v[1] == kernel:
-                return float(v[2]), (float(v[3]) if len(v) >= 4 else None), "profiles/traffic.txt"
+                found = (float(v[2]), float(v[3]) if len(v) >= 4 else None, " ".join(v[4:]) or None)
     except OSError:
-        pass
-    return None, None, None
+        return None, None, None, None
+    if found is None:
+        return None, None, None, None
+    now = kernel_source_hash()
+    if captured != now:
+        return None, None, None, f"stale: profiles/traffic.txt was captured from kernel sources {captured}, the tree is {now}"
+    return (*found, f"profiles/traffic.txt (kernel sources {now})")
 
 
 # ------------------------------------------------------------------------------------------------ arms
@@ -494,6 +585,9 @@ def run_ours(args) -> None:
     value = n_cl_all / (ms_per_step * 1e-3)
     # ---- outside the timed region: per-kernel times (event pair around every kernel) for the roofline of the dominant kernel
     kms = per_kernel_ms(T, ctx, fr, stream)
+    overlap = None
+    if world == 1 and rank == 0 and not args.no_extras:
+        overlap = two_in_flight(T, ctx, geo, arrays, device, min(args.steps, 10), sum(step_ms) / args.steps)
 
     # ---- end to end: pinned host buffers in, pinned host buffers out, every copy inside the timed region.  Frames go
     #      through the library's two-slot pipeline (tmd_decode_host_async): the upload of frame i+1 runs beside the
@@ -505,22 +599,26 @@ def run_ours(args) -> None:
     torch.cuda.empty_cache()
     hcomp = T.make_compressed(h_in)
     houts, keep = [], []
-    for _ in range(T.TMD_HOST_SLOTS):
+    # One rank alone pins an output buffer per pipeline slot (download of frame i beside upload of frame i+1).  With several
+    # ranks on one host that is 15 GB of page-locked memory per rank (123 GB at 8 ranks): they pin ONE output buffer and use
+    # one slot, i.e. upload, decode and download of a rank's frames run one after the other (the line says so in e2e.mode).
+    e2e_slots = T.TMD_HOST_SLOTS if world == 1 else 1
+    for _ in range(e2e_slots):
         hc = torch.empty(n_cl * 16, dtype=torch.uint8, pin_memory=True)
         hb = torch.empty(geo.n_bins + 1, dtype=torch.int32, pin_memory=True)
         keep.append((hc, hb))
         houts.append(T.make_output(hc, hb))
     d2h = keep[0][0].numel() + keep[0][1].numel() * 4
     e2e_steps = max(2, min(args.steps, args.e2e_steps))
-    for s_ in range(T.TMD_HOST_SLOTS):                        # warm-up: allocates the slots' device arenas
+    for s_ in range(e2e_slots):                               # warm-up: allocates the slots' device arenas
         T.tmd_decode_host_async(ctx, hcomp, houts[s_], 0, s_)
-    for s_ in range(T.TMD_HOST_SLOTS):
+    for s_ in range(e2e_slots):
         T.tmd_host_wait(ctx, s_)
     barrier()
     t0 = time.perf_counter()
     for i in range(e2e_steps):
-        T.tmd_decode_host_async(ctx, hcomp, houts[i % T.TMD_HOST_SLOTS], 0, i % T.TMD_HOST_SLOTS)   # waits for the slot's previous frame
-    for s_ in range(T.TMD_HOST_SLOTS):
+        T.tmd_decode_host_async(ctx, hcomp, houts[i % e2e_slots], 0, i % e2e_slots)   # waits for the slot's previous frame
+    for s_ in range(e2e_slots):
         T.tmd_host_wait(ctx, s_)
     e2e_s = time.perf_counter() - t0
     te = torch.tensor([e2e_s], dtype=torch.float64, device=device)
@@ -546,7 +644,7 @@ def run_ours(args) -> None:
         dom = max(kms, key=kms.get)
         alg = kalg.get(dom)
         achieved = alg / (kms[dom] * 1e-3) / 1e9 if alg else None
-        traffic, warp_inst, src = ncu_profile_numbers(dom, args.workload)
+        traffic, warp_inst, observed, src = ncu_profile_numbers(dom, args.workload)
         # second bound: instruction issue.  One warp instruction per scheduler and cycle, 4 schedulers per SM.
         props = torch.cuda.get_device_properties(device)
         sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
@@ -558,7 +656,10 @@ def run_ours(args) -> None:
                       "source": src}
         roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                     "frac": achieved / peak if achieved else None, "traffic": traffic, "traffic_source": src,
-                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kms[dom], "second_bound": second,
+                    "algorithmic_bytes_per_launch": alg, "kernel_ms": kms[dom],
+                    # the second bound as flat keys (nested objects do not survive every reader of this line)
+                    "issue_frac": second["frac"] if second else None, "issue_floor_ms": second["floor_ms"] if second else None,
+                    "bound_observed": observed, "second_bound": second,
                     "note": "kernel timed with an event pair around it in a separate pass after the timed region (same stream, "
                             "same launch configuration)"}
         st = stats(step_ms)
@@ -570,7 +671,9 @@ def run_ours(args) -> None:
                        "sectors_x_rows": "36x152", "bz_tesla": BZ, "l2": "inputs larger than L2, no flush"
                        if alg_total > 400e6 else "L2-resident workload (flag)", "parallelism": f"replicas x{world}"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-                    "mode": "two-slot pipeline, tmd_decode_host_async", "single_frame_ms": 1e3 * e2e_single_s},
+                    "mode": "two-slot pipeline, tmd_decode_host_async" if e2e_slots == 2 else
+                    "one slot per rank (several ranks share the host's pinned memory), tmd_decode_host_async",
+                    "single_frame_ms": 1e3 * e2e_single_s},
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": roofline,
@@ -580,6 +683,8 @@ def run_ours(args) -> None:
         }
         if world == 1 and not args.no_extras:
             other = {}
+            if overlap:
+                other[f"{args.workload}_two_in_flight"] = overlap
             for name in ("c2", "c4"):
                 if name != args.workload:
                     other[name] = side_workload(T, name, device, min(args.steps, 10), peak)
@@ -588,10 +693,14 @@ def run_ours(args) -> None:
             if b:
                 other[f"c1x{BATCH_FRAMES}"] = b
             torch.cuda.empty_cache()
-            z = entropy_workload(T, device, min(args.steps, 10), peak)
+            z = entropy_workload(T, device, min(args.steps, 10), peak, args.workload)
             if z:
                 other["entropy_stage"] = z
+                line["e2e_container"] = z["e2e_container"]      # beside `e2e` (arrays in), which stays the headline e2e
             line["other_workloads"] = other
+        if world > 1:
+            line["legs_skipped"] = ["other_workloads (c2, c4, 64 x c1, two frames in flight, entropy stage): single-rank measurements",
+                                    "cpu_baseline: rank 0 at N = 1 only"]
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_tracks, device, value, not args.no_extras)
         print(json.dumps(line), flush=True)

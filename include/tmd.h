@@ -145,7 +145,6 @@ typedef struct tmd_ctx tmd_ctx;
 #define TMD_TIMING 2u   /* record a CUDA event pair around every kernel (tmd_kernel_times).  The first such call on a
                            context creates the 2 x TMD_MAX_KERNELS events; calls with TMD_TIMING must not run concurrently
                            on one context */
-#define TMD_SERIAL 4u   /* accepted and ignored: every kernel of a call already runs on `cuda_stream`, one after the other */
 #define TMD_MAX_KERNELS 24
 #define TMD_MAX_BATCH 1024 /* frames per tmd_decode_batch call */
 
@@ -326,12 +325,29 @@ int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster
  *                          outside the container is refused on the host (TMD_ERR_CORRUPT).
  *                          The arrays can be handed to tmd_decode on the same stream right away.
  */
+#define TMD_ENTROPY_HEAD_BYTES 1440u /* 64-byte header + 43 plane records of 32 bytes */
 int tmd_entropy_bound(uint32_t n_tracks, uint64_t n_attached, uint64_t n_unattached, uint32_t n_bins, size_t* out_bytes);
 int tmd_entropy_encode_host(const tmd_compressed* in, uint32_t n_bins, void* blob, size_t capacity, size_t* out_bytes);
 int tmd_entropy_sizes(const void* head, size_t head_bytes, uint32_t* n_tracks, uint64_t* n_attached, uint64_t* n_unattached,
                       uint32_t* n_bins, size_t* blob_bytes);
 int tmd_entropy_decode(const void* head, size_t head_bytes, const void* d_blob, size_t blob_bytes, tmd_compressed* out, void* d_err4,
                        void* cuda_stream);
+
+/*
+ * The deployment shape end to end (entropy decoding, then track-model decoding, transfers beside the
+ * kernels): a TMDZ container in HOST memory in, decoded clusters in HOST memory out.  Works like tmd_decode_host_async --
+ * same slots, same three streams, same tmd_host_wait -- but uploads the CONTAINER (about 2.3x smaller than the arrays it
+ * codes), runs tmd_entropy_decode into arrays inside the slot's device arena and tmd_decode right behind it on the same
+ * stream; the compressed arrays never exist in host memory.
+ *   blob / blob_bytes : HOST, the whole container (at least the size its header states); pinned memory makes the copy
+ *                       asynchronous; must stay valid until tmd_host_wait(slot) returns.  Its bin count must be the
+ *                       context's (TMD_ERR_ARG otherwise); a header that is not TMDZ: TMD_ERR_CORRUPT.
+ *   out               : HOST pointers as in tmd_decode_host (clusters sized from tmd_entropy_sizes; workspace ignored).
+ * tmd_host_wait(slot) returns TMD_ERR_CORRUPT if the entropy stage flagged the container (see tmd_entropy_decode); the
+ * output is then unspecified.  TMD_VALIDATE is not accepted (TMD_ERR_ARG).  May be mixed with tmd_decode_host_async calls
+ * on other slots.  The first call on a slot allocates (device arena, a pinned error word, events).
+ */
+int tmd_decode_container_host_async(tmd_ctx* ctx, const void* blob, size_t blob_bytes, tmd_output* out, uint32_t flags, int slot);
 
 #ifdef __cplusplus
 }

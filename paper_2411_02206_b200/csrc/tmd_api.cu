@@ -43,6 +43,8 @@ struct tmd_ctx {
     size_t arena_bytes;
     cudaEvent_t h2d_done, dec_done, d2h_done;
     bool busy;
+    uint32_t* h_err;            // pinned: error word of the slot's last container decode (tmd_decode_container_host_async)
+    bool container;             // the frame in flight came from a container: tmd_host_wait looks at *h_err
   } slots[TMD_HOST_SLOTS];
   cudaStream_t s_h2d, s_dec, s_d2h;
   bool host_ready;
@@ -678,18 +680,50 @@ int tmd_encode_unattached(tmd_ctx* ctx, uint64_t n_unattached, const tmd_cluster
   return TMD_OK;
 }
 
+// the three streams of the host pipeline (uploads, decode, downloads), created on first use
+static int host_streams(tmd_ctx* ctx) {
+  if (!ctx->host_ready) {
+    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
+    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_dec, cudaStreamNonBlocking));
+    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+    ctx->host_ready = true;
+  }
+  return TMD_OK;
+}
+
 // Enqueue one host-to-host decode in slot `slot`: copies in on `s_in`, decode on `s_run`, copies out on `s_out` (the three
 // may be the same stream), ordered by the slot's events.  Does not wait for the result.
-static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot, cudaStream_t s_in,
-                        cudaStream_t s_run, cudaStream_t s_out) {
-  int rc = check_args(ctx, in, out, false);
-  if (rc != TMD_OK) return rc;
+// With `blob` (a TMDZ container in HOST memory) the inputs are not the arrays of `in` but the container: it alone is copied
+// to the device, the entropy stage decodes it into the slot's arrays on `s_run`, and tmd_decode follows on the same stream.
+static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, const void* blob, size_t blob_bytes, tmd_output* out, uint32_t flags,
+                        int slot, cudaStream_t s_in, cudaStream_t s_run, cudaStream_t s_out) {
+  int rc;
+  tmd_compressed counts;                         // container path: the counts of its header, no pointers
+  if (blob) {
+    if (!ctx || !out || !out->bin_offset) return TMD_ERR_ARG;
+    memset(&counts, 0, sizeof(counts));
+    uint32_t z_bins = 0;
+    size_t z_total = 0;
+    rc = tmd_entropy_sizes(blob, blob_bytes, &counts.n_tracks, &counts.n_attached, &counts.n_unattached, &z_bins, &z_total);
+    if (rc != TMD_OK) return rc;
+    if (z_total > blob_bytes || z_total < TMD_ENTROPY_HEAD_BYTES) return TMD_ERR_CORRUPT;
+    if (z_bins != ctx->geo.n_bins) return TMD_ERR_ARG;                      // written for another geometry
+    if (counts.n_attached + counts.n_unattached > TMD_MAX_CLUSTERS) return TMD_ERR_ARG;
+    if ((counts.n_tracks == 0) != (counts.n_attached == 0)) return TMD_ERR_CORRUPT;
+    if (counts.n_attached + counts.n_unattached > 0 && !out->clusters) return TMD_ERR_ARG;
+    blob_bytes = z_total;
+    in = &counts;
+  } else {
+    rc = check_args(ctx, in, out, false);
+    if (rc != TMD_OK) return rc;
+  }
   tmd_ctx::HostSlot& S = ctx->slots[slot];
   if (!S.h2d_done) {
     TMD_CUDA(cudaEventCreateWithFlags(&S.h2d_done, cudaEventDisableTiming));
     TMD_CUDA(cudaEventCreateWithFlags(&S.dec_done, cudaEventDisableTiming));
     TMD_CUDA(cudaEventCreateWithFlags(&S.d2h_done, cudaEventDisableTiming));
   }
+  if (blob && !S.h_err) TMD_CUDA(cudaHostAlloc((void**)&S.h_err, 4, cudaHostAllocDefault));
   const uint32_t n_bins = ctx->geo.n_bins;
   const size_t n_trk = in->n_tracks, n_att = in->n_attached, n_res = n_att - n_trk, n_un = in->n_unattached;
   const Workspace W = layout(n_bins, in->n_tracks, n_att, ctx->n_sm);
@@ -710,6 +744,8 @@ static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out,
   const size_t o_binoff = o;   o += align_up(((size_t)n_bins + 1) * 4);
   const size_t o_probe = o;    o += align_up(out->probe_state ? n_trk * 24 : 0);
   const size_t o_ws = o;       o += W.total;
+  const size_t o_blob = o;     o += align_up(blob ? blob_bytes : 0);
+  const size_t o_err = o;      o += align_up(blob ? 4 : 0);
   if (S.busy) {                                   // the slot's previous frame must have left the arena
     TMD_CUDA(cudaEventSynchronize(S.d2h_done));
     S.busy = false;
@@ -721,8 +757,12 @@ static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out,
     S.arena_bytes = o;
   }
   unsigned char* a = (unsigned char*)S.arena;
-  for (const Seg& s : segs)
-    if (s.bytes) TMD_CUDA(cudaMemcpyAsync(a + s.at, s.src, s.bytes, cudaMemcpyHostToDevice, s_in));
+  if (blob) {
+    TMD_CUDA(cudaMemcpyAsync(a + o_blob, blob, blob_bytes, cudaMemcpyHostToDevice, s_in));
+  } else {
+    for (const Seg& s : segs)
+      if (s.bytes) TMD_CUDA(cudaMemcpyAsync(a + s.at, s.src, s.bytes, cudaMemcpyHostToDevice, s_in));
+  }
   tmd_compressed d = *in;
   const void** dst[] = {(const void**)&d.trk_ncl, (const void**)&d.trk_qpt, (const void**)&d.trk_row0, (const void**)&d.trk_sec0,
                         (const void**)&d.trk_pad0, (const void**)&d.trk_time0, (const void**)&d.a_rowdiff, (const void**)&d.a_secleg,
@@ -741,6 +781,10 @@ static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out,
     TMD_CUDA(cudaEventRecord(S.h2d_done, s_in));
     TMD_CUDA(cudaStreamWaitEvent(s_run, S.h2d_done, 0));
   }
+  if (blob) {   // entropy stage on the decode stream: container -> the slot's arrays (the header is read from the HOST copy)
+    rc = tmd_entropy_decode(blob, TMD_ENTROPY_HEAD_BYTES, a + o_blob, blob_bytes, &d, a + o_err, (void*)s_run);
+    if (rc != TMD_OK) return rc;
+  }
   rc = tmd_decode(ctx, &d, &dout, flags, (void*)s_run);
   if (rc != TMD_OK) return rc;
   if (s_out != s_run) {
@@ -751,6 +795,8 @@ static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out,
   TMD_CUDA(cudaMemcpyAsync(out->bin_offset, dout.bin_offset, ((size_t)n_bins + 1) * 4, cudaMemcpyDeviceToHost, s_out));
   if (out->probe_state && n_trk)
     TMD_CUDA(cudaMemcpyAsync(out->probe_state, dout.probe_state, n_trk * 24, cudaMemcpyDeviceToHost, s_out));
+  if (blob) TMD_CUDA(cudaMemcpyAsync(S.h_err, a + o_err, 4, cudaMemcpyDeviceToHost, s_out));
+  S.container = blob != nullptr;
   TMD_CUDA(cudaEventRecord(S.d2h_done, s_out));
   S.busy = true;
   return TMD_OK;
@@ -759,20 +805,24 @@ static int host_enqueue(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out,
 int tmd_decode_host(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, void* cuda_stream) {
   if (!ctx) return TMD_ERR_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  int rc = host_enqueue(ctx, in, out, flags, 0, st, st, st);
+  int rc = host_enqueue(ctx, in, nullptr, 0, out, flags, 0, st, st, st);
   if (rc != TMD_OK) return rc;
   return tmd_host_wait(ctx, 0);
 }
 
 int tmd_decode_host_async(tmd_ctx* ctx, const tmd_compressed* in, tmd_output* out, uint32_t flags, int slot) {
   if (!ctx || slot < 0 || slot >= TMD_HOST_SLOTS || (flags & TMD_VALIDATE)) return TMD_ERR_ARG;
-  if (!ctx->host_ready) {
-    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
-    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_dec, cudaStreamNonBlocking));
-    TMD_CUDA(cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
-    ctx->host_ready = true;
-  }
-  return host_enqueue(ctx, in, out, flags, slot, ctx->s_h2d, ctx->s_dec, ctx->s_d2h);
+  const int rc_s = host_streams(ctx);
+  if (rc_s != TMD_OK) return rc_s;
+  return host_enqueue(ctx, in, nullptr, 0, out, flags, slot, ctx->s_h2d, ctx->s_dec, ctx->s_d2h);
+}
+
+int tmd_decode_container_host_async(tmd_ctx* ctx, const void* blob, size_t blob_bytes, tmd_output* out, uint32_t flags, int slot) {
+  if (!ctx || !blob || slot < 0 || slot >= TMD_HOST_SLOTS || (flags & TMD_VALIDATE)) return TMD_ERR_ARG;
+  if (blob_bytes < TMD_ENTROPY_HEAD_BYTES) return TMD_ERR_ARG;
+  const int rc = host_streams(ctx);
+  if (rc != TMD_OK) return rc;
+  return host_enqueue(ctx, nullptr, blob, blob_bytes, out, flags, slot, ctx->s_h2d, ctx->s_dec, ctx->s_d2h);
 }
 
 int tmd_host_wait(tmd_ctx* ctx, int slot) {
@@ -781,6 +831,7 @@ int tmd_host_wait(tmd_ctx* ctx, int slot) {
   if (!S.busy) return TMD_OK;
   TMD_CUDA(cudaEventSynchronize(S.d2h_done));
   S.busy = false;
+  if (S.container && *S.h_err) return TMD_ERR_CORRUPT;      // the entropy stage found the container damaged
   return TMD_OK;
 }
 
@@ -810,6 +861,7 @@ int tmd_destroy(tmd_ctx* ctx) {
     if (S.busy) cudaEventSynchronize(S.d2h_done);
     if (S.arena) cudaFree(S.arena);
     if (S.h2d_done) { cudaEventDestroy(S.h2d_done); cudaEventDestroy(S.dec_done); cudaEventDestroy(S.d2h_done); }
+    if (S.h_err) cudaFreeHost(S.h_err);
   }
   if (ctx->host_ready) { cudaStreamDestroy(ctx->s_h2d); cudaStreamDestroy(ctx->s_dec); cudaStreamDestroy(ctx->s_d2h); }
   if (ctx->d_rows) cudaFree(ctx->d_rows);

@@ -46,6 +46,7 @@ struct ZArgs {
   ZPlane pl[Z_PLANES];
 };
 static_assert(sizeof(ZArgs) < 3800, "kernel parameter space");
+static_assert(Z_HEADER + Z_PLANE * Z_PLANES == TMD_ENTROPY_HEAD_BYTES, "include/tmd.h states the size of header + plane directory");
 
 // One CTA assembles Z_CHUNK_BYTES of one output array: warp wi decodes block (chunk * (8 / w) + wi / w) of byte plane
 // (wi mod w) into shared memory, then the CTA interleaves the planes into elements and writes them with coalesced stores.

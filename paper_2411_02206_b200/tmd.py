@@ -19,7 +19,6 @@ TMD_OK, TMD_ERR_ARG, TMD_ERR_ALIGN, TMD_ERR_WORKSPACE, TMD_ERR_CUDA, TMD_ERR_COR
 TMD_NOALLOC_MAX_BINS = 8192
 TMD_VALIDATE = 1
 TMD_TIMING = 2
-TMD_SERIAL = 4
 TMD_MAX_KERNELS = 24
 TMD_MAX_BATCH = 1024
 TMD_HOST_SLOTS = 2
@@ -84,6 +83,8 @@ def lib() -> C.CDLL:
                                           C.c_size_t, C.c_void_p]
         L.tmd_decode_host_async.argtypes = [C.c_void_p, C.POINTER(tmd_compressed), C.POINTER(tmd_output), C.c_uint32, C.c_int]
         L.tmd_host_wait.argtypes = [C.c_void_p, C.c_int]
+        L.tmd_decode_container_host_async.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(tmd_output), C.c_uint32, C.c_int]
+        L.tmd_decode_container_host_async.restype = C.c_int
         L.tmd_encode_unattached_workspace_bytes.argtypes = [C.c_void_p, C.c_uint64, C.POINTER(C.c_size_t)]
         L.tmd_encode_unattached_workspace_bytes.restype = C.c_int
         L.tmd_encode_unattached.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.POINTER(tmd_compressed), C.c_void_p, C.c_size_t, C.c_void_p]
@@ -203,6 +204,13 @@ def tmd_decode_host(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int 
 def tmd_decode_host_async(ctx: int, comp: tmd_compressed, out: tmd_output, flags: int = 0, slot: int = 0) -> None:
     """Enqueue upload + decode + download of one time frame (pinned HOST pointers) in pipeline slot `slot`; returns at once."""
     _check(lib().tmd_decode_host_async(ctx, C.byref(comp), C.byref(out), flags, slot))
+
+
+def tmd_decode_container_host_async(ctx: int, blob, out: tmd_output, flags: int = 0, slot: int = 0) -> None:
+    """Enqueue upload of a TMDZ container (HOST uint8 array / pinned tensor) + entropy decode + track-model decode + download of
+    the clusters in pipeline slot `slot`; returns at once.  tmd_host_wait(slot) raises TMD_ERR_CORRUPT for a damaged container."""
+    n = int(blob.size if isinstance(blob, np.ndarray) else blob.numel())
+    _check(lib().tmd_decode_container_host_async(ctx, _ptr(blob), n, C.byref(out), flags, slot))
 
 
 def tmd_host_wait(ctx: int, slot: int = 0) -> None:

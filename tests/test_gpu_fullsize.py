@@ -229,3 +229,47 @@ def test_whole_chunks_in_one_bin_at_the_full_frame_chunk_size():
     c = degenerate_same_bin(geo, ncl, 62, n_un=10_000)
     assert c.n_attached >= 97_000_000
     _compare_with_oracle(geo, c, "one bin, shift 15")
+
+
+def test_full_c2_container_in_clusters_out():
+    """The whole chain at time-frame size: oracle encoder -> ORACLE rANS coder -> container in pinned host memory ->
+    tmd_decode_container_host_async (upload, GPU entropy decode, track-model decode, download) -> every record and bin offset
+    against orc_decode.  No input of the library comes from the library."""
+    import torch
+    from oracle import tmd_ans as ANS, tmd_oracle as O
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs import build_geometry, timeframe as tf
+    from tmd_inputs.layout import CLUSTER_DTYPE
+
+    if _host_gb_available() < 12:
+        pytest.skip(f"needs 12 GB of host memory for the oracle side, {_host_gb_available():.0f} GB available")
+    dev = torch.device("cuda", 0)
+    geo = build_geometry(36)
+    mk, n_un, single = tf.WORKLOADS["c2"]
+    cfg = mk()
+    truth = tf.generate_truth(cfg, geo, dev, batch=2_000_000)
+    un = tf.generate_unattached_truth(geo, n_un, cfg.seed, dev, "inv_x", single)
+    comp = O.encode(geo, BZ, truth.trk_ncl.cpu().numpy().view(np.uint16), truth.trk_qptf.cpu().numpy(),
+                    truth.att.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1), truth.leg.cpu().numpy(),
+                    un.cpu().numpy().view(CLUSTER_DTYPE).reshape(-1))
+    del truth, un
+    torch.cuda.empty_cache()
+    blob = torch.from_numpy(ANS.encode_container(comp)).pin_memory()
+    assert blob.numel() < comp.nbytes() / 1.5                      # it is a compressed container
+    want_cl, want_bo, _ = O.decode(geo, BZ, comp)
+    n = comp.n_attached + comp.n_unattached
+    hc = torch.full((n * 16,), 0xEE, dtype=torch.uint8).pin_memory()
+    hb = torch.zeros(geo.n_bins + 1, dtype=torch.int32).pin_memory()
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        T.tmd_decode_container_host_async(ctx, blob, T.make_output(hc, hb), 0, 0)
+        T.tmd_host_wait(ctx, 0)
+    finally:
+        T.tmd_destroy(ctx)
+    assert np.array_equal(hb.numpy().view(np.uint32), want_bo)
+    got = hc.numpy().view(CLUSTER_DTYPE)
+    if got.tobytes() != want_cl.tobytes():
+        for f in want_cl.dtype.names:
+            d = np.nonzero(got[f] != want_cl[f])[0]
+            assert d.size == 0, f"{d.size} records differ in {f}; first at {int(d[0])}"
+        raise AssertionError("bytes differ")

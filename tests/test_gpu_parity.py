@@ -242,14 +242,14 @@ def test_pipelined_host_entry_points_match():
         T.tmd_destroy(ctx)
 
 
-def test_serial_and_timing_flags_do_not_change_the_result():
-    # TMD_SERIAL (one stream) and TMD_TIMING (event pairs around the kernels) are the modes bench.py's per-kernel pass uses
+def test_timing_and_validate_flags_do_not_change_the_result():
+    # TMD_TIMING (event pairs around the kernels) is the mode bench.py's per-kernel pass uses
     import torch
     from paper_2411_02206_b200 import tmd as T
     geo = build_geometry(36)
     c = random_compressed(geo, 5000, 60_000, 51, max_ncl=180)
     want = O.decode(geo, BZ, c)
-    for flags in (T.TMD_SERIAL, T.TMD_TIMING, T.TMD_SERIAL | T.TMD_TIMING, T.TMD_SERIAL | T.TMD_VALIDATE):
+    for flags in (T.TMD_TIMING, T.TMD_VALIDATE, T.TMD_TIMING | T.TMD_VALIDATE):
         assert_same(gpu_decode(geo, BZ, c, flags=flags), want)
     ctx = T.tmd_create(geo, BZ)
     try:
@@ -259,7 +259,7 @@ def test_serial_and_timing_flags_do_not_change_the_result():
         n = c.n_attached + c.n_unattached
         out = T.make_output(torch.empty(n * 16, dtype=torch.uint8, device="cuda"), torch.empty(geo.n_bins + 1, dtype=torch.int32, device="cuda"),
                             torch.empty(T.tmd_workspace_bytes(ctx, c.n_tracks, c.n_attached, c.n_unattached), dtype=torch.uint8, device="cuda"))
-        T.tmd_decode(ctx, T.make_compressed(dev), out, T.TMD_TIMING | T.TMD_SERIAL, torch.cuda.current_stream().cuda_stream)
+        T.tmd_decode(ctx, T.make_compressed(dev), out, T.TMD_TIMING, torch.cuda.current_stream().cuda_stream)
         times = dict(T.tmd_kernel_times(ctx))
         assert T.tmd_last_launch_count(ctx) == len(times) == 12
         assert {"track_decode", "rank", "scatter", "unattached", "bin_offsets"} <= set(times) and all(v >= 0 for v in times.values())
@@ -530,3 +530,65 @@ def test_entropy_decode_edge_cases_and_library_encoder():
     out, err = _gpu_entropy_decode(blob)                    # the context survived all of the above
     assert err == 0
     _assert_arrays_equal(out, c)
+
+
+def test_container_host_entry_point_matches_oracle(phys_case):
+    # The deployment shape: a TMDZ container in host memory in, clusters in host memory out, through
+    # tmd_decode_container_host_async.  The container is written by the ORACLE (oracle encoder -> oracle rANS coder) and the
+    # result must be orc_decode's, record for record.  Frames alternate between the two pipeline slots, mixed with the
+    # array-input entry point on the other slot.
+    import torch
+    from oracle import tmd_ans as ANS
+    from paper_2411_02206_b200 import tmd as T
+    from tmd_inputs.layout import CLUSTER_DTYPE, COMPRESSED_FIELDS
+    from gpu_util import _as_torch
+    name, geo, ev, comp = phys_case
+    blob = torch.from_numpy(ANS.encode_container(comp)).pin_memory()
+    want_cl, want_bo, _ = O.decode(geo, BZ, comp)
+    n = comp.n_attached + comp.n_unattached
+    assert T.tmd_entropy_sizes(blob.numpy()[:64])[:3] == (comp.n_tracks, comp.n_attached, comp.n_unattached)
+    ctx = T.tmd_create(geo, BZ)
+    try:
+        outs = [(torch.full((n * 16,), 0xEE, dtype=torch.uint8).pin_memory(), torch.zeros(geo.n_bins + 1, dtype=torch.int32).pin_memory())
+                for _ in range(3)]
+        h_in = {k: _as_torch(np.ascontiguousarray(getattr(comp, k))).pin_memory() for k in COMPRESSED_FIELDS}
+        T.tmd_decode_container_host_async(ctx, blob, T.make_output(*outs[0]), 0, 0)
+        T.tmd_decode_host_async(ctx, T.make_compressed(h_in), T.make_output(*outs[1]), 0, 1)       # arrays in, other slot
+        T.tmd_decode_container_host_async(ctx, blob, T.make_output(*outs[2]), 0, 0)               # waits for slot 0's first frame
+        for s_ in range(T.TMD_HOST_SLOTS):
+            T.tmd_host_wait(ctx, s_)
+        for hc, hb in outs:
+            assert np.array_equal(hb.numpy().view(np.uint32), want_bo)
+            assert hc.numpy().view(CLUSTER_DTYPE).tobytes() == want_cl.tobytes()
+        if name == "c0":
+            # a damaged container is reported by tmd_host_wait; a container of another geometry, a non-container and the
+            # synchronising flag are refused at the call
+            bad = blob.clone()
+            rec = bad.numpy()[64:96]
+            b_off = int(rec[24:32].view(np.uint64)[0])
+            s0 = int(bad.numpy()[b_off:b_off + 4].view(np.uint32)[0])
+            bad.numpy()[s0 + 4 * 32 + 10] ^= 0x04
+            bad = bad.pin_memory()
+            T.tmd_decode_container_host_async(ctx, bad, T.make_output(*outs[0]), 0, 1)
+            with pytest.raises(T.TmdError) as e:
+                T.tmd_host_wait(ctx, 1)
+            assert e.value.status == T.TMD_ERR_CORRUPT
+            T.tmd_decode_container_host_async(ctx, blob, T.make_output(*outs[0]), 0, 1)          # the slot is usable again
+            T.tmd_host_wait(ctx, 1)
+            assert outs[0][0].numpy().view(CLUSTER_DTYPE).tobytes() == want_cl.tobytes()
+            with pytest.raises(T.TmdError) as e:
+                T.tmd_decode_container_host_async(ctx, blob, T.make_output(*outs[0]), T.TMD_VALIDATE, 0)
+            assert e.value.status == T.TMD_ERR_ARG
+            junk = torch.zeros(4096, dtype=torch.uint8).pin_memory()
+            with pytest.raises(T.TmdError) as e:
+                T.tmd_decode_container_host_async(ctx, junk, T.make_output(*outs[0]), 0, 0)
+            assert e.value.status == T.TMD_ERR_CORRUPT
+            other = T.tmd_create(build_geometry(36 if geo.n_sectors_out == 2 else 2), BZ)
+            try:
+                with pytest.raises(T.TmdError) as e:
+                    T.tmd_decode_container_host_async(other, blob, T.make_output(*outs[0]), 0, 0)
+                assert e.value.status == T.TMD_ERR_ARG
+            finally:
+                T.tmd_destroy(other)
+    finally:
+        T.tmd_destroy(ctx)

@@ -16,15 +16,6 @@ def truth_to_event(tr: tf.Truth) -> ph.Event:
                     att=att, leg=tr.leg.cpu().numpy(), un=np.zeros(0, CLUSTER_DTYPE))
 
 
-def unattached_to_compressed(u: dict, n_bins: int) -> Compressed:
-    n = int(u["u_qtot"].shape[0])
-    c = Compressed.empty(0, 0, n, n_bins)
-    for k, v in u.items():
-        a = v.cpu().numpy()
-        getattr(c, k)[:] = a.view(getattr(c, k).dtype)
-    return c
-
-
 def test_truth_round_trips_through_the_oracle_codec():
     geo = build_geometry(36)
     for cfg in (ph.config2_like(1500, 0, seed=3), ph.config4_like(6000, 0, seed=5)):
@@ -50,16 +41,18 @@ def test_workload_shapes():
     assert 25 < ncl.mean() < 50 and ncl.max() > 300 and ncl.min() == 1             # geometric(40) + long loopers
 
 
-def test_unattached_generator_is_a_valid_compressed_stream():
+def test_unattached_truth_generator_through_the_oracle_codec():
     geo = build_geometry(36)
-    u = tf.generate_unattached(geo, 200_000, seed=3, device="cpu")
-    c = unattached_to_compressed(u, geo.n_bins)
+    un = tf.generate_unattached_truth(geo, 200_000, 3, "cpu").numpy().view(CLUSTER_DTYPE).reshape(-1)
+    assert abs(len(un) - 200_000) < 5000
+    c = O.encode(geo, BZ, np.zeros(0, np.uint16), np.zeros(0, np.float32), np.zeros(0, CLUSTER_DTYPE), np.zeros(0, np.uint8), un)
     c.check_shapes()
-    assert abs(c.n_unattached - 200_000) < 5000 and int(c.u_bin_count.sum()) == c.n_unattached
+    assert int(c.u_bin_count.sum()) == c.n_unattached == len(un)
     cl, bo, _ = O.decode(geo, BZ, c)
-    # density ~ 1/x(row); decoded times ascend inside a bin (sorted)
+    # density ~ 1/x(row); decoded times ascend inside a bin (sorted by the encoder); pads inside the row
     per_row = np.bincount(cl["row"], minlength=152)
     assert per_row[:10].mean() > 2.0 * per_row[-10:].mean()
     same = (cl["row"][1:] == cl["row"][:-1]) & (cl["sector"][1:] == cl["sector"][:-1])
     assert np.all(cl["time"][1:][same] >= cl["time"][:-1][same])
     assert cl["time"].max() < (1 << 24)
+    assert np.all(cl["pad"] < geo.row_npads[cl["row"]].astype(np.int64) * 64)

@@ -8,9 +8,8 @@ Two generators, neither containing arithmetic of the track-model codec:
   ops so that 2-3 M tracks / 240 M clusters are generated on the GPU in seconds.  Output = cluster truth of the
   ATTACHED clusters (g-ordered 16-byte records + leg index + per-track length and curvature).  It becomes the compressed
   SoA through an encoder: the oracle's in tests, the library's `tmd_encode_attached` in bench.py.
-* `generate_unattached` -- the UNATTACHED clusters directly in the compressed domain: per-bin counts Poisson around a
-  1/x(row) density, time differences as exponential gaps (sorted times), pad differences drawn as the difference of two
-  independent uniform pads of the row (the decoded pads are then a random walk mod 2^16: valid input, same value widths).
+* `generate_unattached_truth` -- the UNATTACHED clusters in the cluster domain (per-bin counts Poisson around a 1/x(row)
+  density, pad uniform over the row, time uniform over the frame, arbitrary order inside a bin): truth for an encoder.
 
 Random numbers come from a seeded torch.Generator on the target device (CPU and CUDA streams differ; a run is
 reproducible per device).
@@ -218,40 +217,6 @@ def generate_truth(cfg: EventConfig, geo: Geometry, device="cpu", batch: int = 4
         need -= good.numel()
         del tid, leg, sec, row, P, T, m, sel
     return Truth(*(torch.cat(c) for c in zip(*parts)))
-
-
-def generate_unattached(geo: Geometry, n_unattached: int, seed: int, device="cpu", law: str = "inv_x", single_event: bool = False) -> dict:
-    """Unattached clusters of one time frame, directly in the compressed domain.
-    Returns dict name -> tensor for the seven u_* value arrays and u_bin_count; the total is Poisson around n_unattached."""
-    device = torch.device(device)
-    gen = torch.Generator(device=device)
-    gen.manual_seed(seed * 7919 + 13)
-    n_bins = geo.n_bins
-    w = np.ones(n_bins) if law == "uniform" else np.tile(1.0 / geo.row_x_f64, geo.n_sectors_out)
-    mean = torch.as_tensor(n_unattached * w / w.sum(), dtype=torch.float64, device=device)
-    counts = torch.poisson(mean, generator=gen).to(torch.int64)
-    n = int(counts.sum())
-    bins = torch.repeat_interleave(torch.arange(n_bins, device=device), counts)
-    start = torch.cumsum(counts, 0) - counts
-    first = torch.zeros(n, dtype=torch.bool, device=device)
-    first[start[counts > 0]] = True
-    row = bins % geo.n_rows
-    width = torch.as_tensor(geo.row_npads.astype(np.int64) * 64, device=device)[row]        # pad codes in the row
-    span = (500.0 if single_event else float(TF_NBINS)) * 64.0                                  # time codes covered by a bin
-    base = 2000.0 * 64.0 if single_event else 0.0
-    gap_mean = span / torch.clamp_min(counts, 1).to(torch.float64)[bins]
-    gaps = torch.floor(-gap_mean * torch.log(1.0 - torch.rand(n, generator=gen, device=device, dtype=torch.float64)))
-    timediff = torch.where(first, gaps + base, gaps).to(torch.int64) & 0xFFFFFFFF
-    p1 = (torch.rand(n, generator=gen, device=device, dtype=torch.float64) * width).to(torch.int64)
-    p2 = (torch.rand(n, generator=gen, device=device, dtype=torch.float64) * width).to(torch.int64)
-    paddiff = torch.where(first, p1, p1 - p2) & 0xFFFF
-    qtot, qmax, sigpad, sigtime, flags = _copy_through(gen, n, device)
-    return {
-        "u_qtot": qtot.to(torch.int16), "u_qmax": qmax.to(torch.int16), "u_flags": flags.to(torch.uint8),
-        "u_sigpad": sigpad.to(torch.uint8), "u_sigtime": sigtime.to(torch.uint8),
-        "u_paddiff": paddiff.to(torch.int16), "u_timediff": timediff.to(torch.int32),
-        "u_bin_count": counts.to(torch.int32),
-    }
 
 
 def generate_unattached_truth(geo: Geometry, n_unattached: int, seed: int, device="cpu", law: str = "inv_x",
