@@ -117,6 +117,9 @@ __global__ void __launch_bounds__(Z_THREADS) k_entropy_decode(const __grid_const
     x = reinterpret_cast<const uint32_t*>(blk)[lane];
     words = reinterpret_cast<const uint16_t*>(blk + 4 * Z_LANES);
     max_words = (s1 - s0 - 4 * Z_LANES) / 2;
+    // the whole block into the L2 now: lane l asks for line l of every 4 KB (a block is at most 16.1 KB).  2.31 -> 2.19 ms on a
+    // full c2 container (profiles/r03_entropy_experiments.md)
+    for (uint32_t o = lane * 128u; o < s1 - s0; o += 4096u) asm volatile("prefetch.global.L2 [%0];" ::"l"(blk + o));
   }
   // The words the warp will read next sit in two registers per lane (a 64-word window starting at `base`): a lane takes
   // its word with a shuffle, and the window is refilled 32 words ahead of its use, so no global-memory latency is on the
